@@ -1,0 +1,95 @@
+/*
+ * elpa2_bt.h -- C ABI of the B200-native stage-2 eigenvector back-transformation of ELPA2
+ * (arxiv 2002.10991, Eq. 6d; citations are "PAPER.md:<line>" of the extracted paper text,
+ * "R<n>" are the readings listed in DESIGN.md).
+ *
+ * The operation (Eq. 6d, Eq. 8): given the Householder
+ * reflectors H(s,k) = I - tau v v^H produced by bulge-chasing a band matrix of semi-bandwidth nbw
+ * to tridiagonal form, overwrite the N x nev block q of tridiagonal-basis
+ * eigenvectors with
+ *
+ *      q  <-  H(0,0) H(0,1) ... H(0,K(0)-1) H(1,0) ... H(N-2,0) q ,
+ *
+ * i.e. the reflector generated LAST is applied FIRST ("the reverse of the order in which they
+ * are generated").  tau is used as stored (not conjugated); the dot product
+ * is v^H x (R2).  Sweep s = 0..N-2 (the paper's stage i = s+1) has K(s) = ceil((N-1-s)/nbw)
+ * chase blocks k (the paper's sweep j = k+1); reflector (s,k) acts on rows
+ * r0 = s+1+k*nbw .. min(s+(k+1)*nbw, N-1) (0-based) (R1, R3).
+ *
+ * Reflector layout (sweep-major, generation order; "stored in a separate array"):
+ *   slot g(s,k) = elpa2_hh_offset(N,nbw,s) + k;   tau at hh_tau[g];   v at hh_v[g*nbw + r],
+ *   r = 0..nbw-1, with hh_v[g*nbw] == 1 stored explicitly and entries r >= L equal to ZERO (R8).
+ *   tau == 0 marks an identity slot.  The producer guarantees v[0] == 1 and the zero padding.
+ *
+ * q: column-major, element (r, j) at q[r + j*ldq], 0 <= r < N, 0 <= j < nev, updated in place.
+ * Complex data is interleaved (re, im) doubles (C99 double complex / std::complex<double>).
+ *
+ * Ownership and execution: the caller owns every buffer.  hh_v, hh_tau and q are DEVICE pointers
+ * valid on the current CUDA device; hh_* are read-only.  The call enqueues work on `stream`
+ * (a cudaStream_t passed as void*; NULL = the legacy default stream), returns without
+ * synchronising the host, and allocates nothing (keep data on the device, no
+ * implicit synchronisation).  There is no CPU fallback: without a CUDA device every compute call
+ * fails with the cudaError_t of the launch.
+ *
+ * Return value: 0 on success; -i if the i-th argument (1-based: N=1, nbw=2, nev=3, hh_v=4,
+ * hh_tau=5, q=6, ldq=7, stream=8) is invalid; > 0 is the cudaError_t of a failed launch.
+ * Invalid: N < 0; nbw not in {32, 64, 128} ("32, 64, and 128 being the recommended
+ * choices"); nev < 0; a NULL pointer when there is work to do; ldq < max(N,1); a q or hh_v pointer
+ * that is not aligned to its element size, hh_v not 16-byte aligned (bulk-copy requirement).
+ * N <= 1 or nev == 0 is success with no work.  Nothing is printed, no errno, no exceptions.
+ */
+#ifndef ELPA2_BT_H
+#define ELPA2_BT_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* FP64 real.  hh_v: G*nbw doubles, hh_tau: G doubles, q: ldq*nev doubles (all device). */
+int elpa2_trans_ev_tridi_to_band_d(int64_t N, int nbw, int64_t nev,
+                                   const double *hh_v, const double *hh_tau,
+                                   double *q, int64_t ldq, void *stream);
+
+/* FP64 complex, interleaved (re, im).  hh_v: G*nbw complex, hh_tau: G complex, q: ldq*nev complex
+ * (all device; ldq counts complex elements). */
+int elpa2_trans_ev_tridi_to_band_z(int64_t N, int nbw, int64_t nev,
+                                   const void *hh_v, const void *hh_tau,
+                                   void *q, int64_t ldq, void *stream);
+
+/* Same operation with HOST buffers (pageable or pinned): copies hh_v, hh_tau and q to the device,
+ * runs the kernel, copies q back and synchronises (the paper's steps 1-5).
+ * Device scratch is allocated on first use and cached (grow-only).  is_complex = 0 / 1.
+ * Returns like the calls above (argument positions of the _d/_z signature). */
+int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_t nev,
+                                      const void *hh_v, const void *hh_tau,
+                                      void *q, int64_t ldq);
+
+/* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */
+int64_t elpa2_hh_count(int64_t N, int nbw);
+/* first slot of sweep s (s in [0, N-1]; s = N-1 gives G); -1 if out of range */
+int64_t elpa2_hh_offset(int64_t N, int nbw, int64_t s);
+/* K(s), 0 if s is out of range */
+int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
+
+/* Kernels launched by the last successful compute call of this thread's library state (for
+ * bench.py's "gpu_launches"), and a selector for A/B runs: variant 0 = default (fastest),
+ * 1 = simple shared-memory-window kernel (correctness baseline).  Returns the previous variant
+ * or -1 if `variant` is unknown. */
+int elpa2_bt_last_launch_count(void);
+int elpa2_bt_set_variant(int variant);
+
+const char *elpa2_bt_version(void);
+
+/* Measurement aid (synchronous; allocates and frees a small device buffer): sustained FP64 ALU
+ * throughput of the current device in TFLOP/s, the denominator of the "alu" roofline.
+ * kind 0 = DFMA, 1 = DMMA (mma.sync m8n8k4 f64), 2 = DMMA on even warps + DFMA on odd warps.
+ * Each launch runs `iters` x 64 FMA per thread on 4 x 512 threads per SM; `reps` launches are
+ * timed with CUDA events.  Returns 0, -1 on a bad argument, or a cudaError_t. */
+int elpa2_bt_probe_fp64(int kind, int iters, int reps, double *tflops);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ELPA2_BT_H */

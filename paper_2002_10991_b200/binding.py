@@ -1,0 +1,166 @@
+"""Thin ctypes binding of the C-ABI library declared in ``include/elpa2_bt.h``.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels behind the C ABI.
+torch is used for device memory and streams, nothing else.  There is no CPU fallback: if the
+library is missing the import of any entry point raises, loudly.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libelpa2_bt.so")
+SOURCES = [os.path.join(_HERE, "csrc", f) for f in ("elpa2_bt.cu", "fp64_probe.cu")]
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+              "-shared", "-Xcompiler", "-fPIC"]
+
+_lib = None
+
+EXPORTS = (
+    "elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z",
+    "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
+    "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
+)
+
+
+def build(force: bool = False) -> str:
+    """Compile the CUDA library in-tree with nvcc for sm_100a (no GPU needed)."""
+    import subprocess
+
+    deps = SOURCES + [os.path.join(_HERE, "csrc", f) for f in os.listdir(os.path.join(_HERE, "csrc"))]
+    newest = max(os.path.getmtime(p) for p in deps)
+    if force or not os.path.exists(LIB_PATH) or os.path.getmtime(LIB_PATH) < newest:
+        nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+        subprocess.run([nvcc, *NVCC_FLAGS, "-o", LIB_PATH, *SOURCES], check=True)
+    return LIB_PATH
+
+
+def lib() -> ctypes.CDLL:
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(
+                f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        i64, i32, vp = ctypes.c_int64, ctypes.c_int, ctypes.c_void_p
+        for nm in ("elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z"):
+            getattr(L, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64, vp]
+            getattr(L, nm).restype = i32
+        L.elpa2_trans_ev_tridi_to_band_host.argtypes = [i32, i64, i32, i64, vp, vp, vp, i64]
+        L.elpa2_trans_ev_tridi_to_band_host.restype = i32
+        L.elpa2_hh_count.argtypes = [i64, i32]
+        L.elpa2_hh_count.restype = i64
+        L.elpa2_hh_offset.argtypes = [i64, i32, i64]
+        L.elpa2_hh_offset.restype = i64
+        L.elpa2_hh_blocks.argtypes = [i64, i32, i64]
+        L.elpa2_hh_blocks.restype = i32
+        L.elpa2_bt_last_launch_count.argtypes = []
+        L.elpa2_bt_last_launch_count.restype = i32
+        L.elpa2_bt_set_variant.argtypes = [i32]
+        L.elpa2_bt_set_variant.restype = i32
+        L.elpa2_bt_version.argtypes = []
+        L.elpa2_bt_version.restype = ctypes.c_char_p
+        L.elpa2_bt_probe_fp64.argtypes = [i32, i32, i32, ctypes.POINTER(ctypes.c_double)]
+        L.elpa2_bt_probe_fp64.restype = i32
+        _lib = L
+    return _lib
+
+
+class Elpa2BtError(RuntimeError):
+    def __init__(self, rc: int):
+        self.rc = rc
+        what = f"argument {-rc} invalid" if rc < 0 else f"cudaError_t {rc}"
+        super().__init__(f"elpa2_trans_ev_tridi_to_band failed: {what}")
+
+
+def hh_count(N: int, nbw: int) -> int:
+    return lib().elpa2_hh_count(N, nbw)
+
+
+def hh_offset(N: int, nbw: int, s: int) -> int:
+    return lib().elpa2_hh_offset(N, nbw, s)
+
+
+def hh_blocks(N: int, nbw: int, s: int) -> int:
+    return lib().elpa2_hh_blocks(N, nbw, s)
+
+
+def version() -> str:
+    return lib().elpa2_bt_version().decode()
+
+
+def set_variant(variant: int) -> int:
+    return lib().elpa2_bt_set_variant(variant)
+
+
+def last_launch_count() -> int:
+    return lib().elpa2_bt_last_launch_count()
+
+
+def probe_fp64(kind: int, iters: int = 4096, reps: int = 20) -> float:
+    out = ctypes.c_double(0.0)
+    rc = lib().elpa2_bt_probe_fp64(kind, iters, reps, ctypes.byref(out))
+    if rc != 0:
+        raise Elpa2BtError(rc)
+    return out.value
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        import torch
+
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def trans_ev_tridi_to_band_raw(cplx: bool, N: int, nbw: int, nev: int, hh_v_ptr: int, hh_tau_ptr: int,
+                               q_ptr: int, ldq: int, stream_ptr: int) -> int:
+    """The C call itself, on raw device addresses; returns the C return code."""
+    fn = lib().elpa2_trans_ev_tridi_to_band_z if cplx else lib().elpa2_trans_ev_tridi_to_band_d
+    return fn(N, nbw, nev, hh_v_ptr, hh_tau_ptr, q_ptr, ldq, stream_ptr)
+
+
+def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> None:
+    """q <- Q2 q in place (Eq. 6d).  ``q``: CUDA tensor of shape (N, nev), float64 or complex128,
+    stored column-major (``q.stride(0) == 1``; ldq = ``q.stride(1)``).  ``hh_v`` (G, nbw) and
+    ``hh_tau`` (G,) contiguous CUDA tensors of the same dtype, layout per include/elpa2_bt.h."""
+    import torch
+
+    if not (q.is_cuda and hh_v.is_cuda and hh_tau.is_cuda):
+        raise ValueError("device tensors required (use trans_ev_tridi_to_band_host for numpy arrays)")
+    cplx = q.dtype == torch.complex128
+    if q.dtype not in (torch.float64, torch.complex128) or hh_v.dtype != q.dtype or hh_tau.dtype != q.dtype:
+        raise ValueError("float64 or complex128 throughout")
+    if q.dim() != 2 or q.shape[0] != N or (q.shape[0] > 1 and q.stride(0) != 1):
+        raise ValueError("q must be (N, nev) column-major")
+    nev = q.shape[1]
+    ldq = q.stride(1) if nev > 1 else max(N, 1)
+    if not (hh_v.is_contiguous() and hh_tau.is_contiguous()):
+        raise ValueError("hh_v / hh_tau must be contiguous")
+    rc = trans_ev_tridi_to_band_raw(cplx, N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q.data_ptr(),
+                                    ldq, _stream_ptr(stream))
+    if rc != 0:
+        raise Elpa2BtError(rc)
+
+
+def trans_ev_tridi_to_band_host(N: int, nbw: int, hh_v, hh_tau, q) -> None:
+    """Same with HOST numpy arrays (q Fortran-ordered (N, nev), updated in place); the library
+    copies to the device, runs the kernel and copies back (synchronous)."""
+    import numpy as np
+
+    cplx = np.iscomplexobj(q)
+    dt = np.complex128 if cplx else np.float64
+    if q.dtype != dt or hh_v.dtype != dt or hh_tau.dtype != dt:
+        raise ValueError("float64 or complex128 throughout")
+    if q.ndim != 2 or q.shape[0] != N or (N > 1 and q.strides[0] != q.itemsize):
+        raise ValueError("q must be (N, nev) column-major")
+    nev = q.shape[1]
+    ldq = q.strides[1] // q.itemsize if nev > 1 else max(N, 1)
+    if nev > 1 and not q.flags.f_contiguous:
+        raise ValueError("host q must be Fortran-contiguous (ldq == N)")
+    rc = lib().elpa2_trans_ev_tridi_to_band_host(int(cplx), N, nbw, nev, hh_v.ctypes.data, hh_tau.ctypes.data,
+                                                 q.ctypes.data, ldq)
+    if rc != 0:
+        raise Elpa2BtError(rc)

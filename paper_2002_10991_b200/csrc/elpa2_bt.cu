@@ -1,0 +1,206 @@
+// elpa2_bt.cu -- C-ABI entry points of include/elpa2_bt.h: argument validation, launch planning,
+// host-buffer wrapper and the FP64 peak probe.  All arithmetic of the path is in the kernels
+// (bt_window.cuh, bt_simple.cuh).  No torch types, no CPU fallback.
+#include "../../include/elpa2_bt.h"
+
+#include <cuda_runtime.h>
+
+#include <mutex>
+
+#include "bt_simple.cuh"
+#include "bt_window.cuh"
+
+using namespace elpa2bt;
+
+namespace {
+
+int g_variant = 0;
+thread_local int g_last_launches = 0;
+std::mutex g_mu;
+
+int lg_of(int nbw) { return nbw == 32 ? 5 : nbw == 64 ? 6 : nbw == 128 ? 7 : -1; }
+
+int sm_count()
+{
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0, v = 0;
+        if (cudaGetDevice(&dev) == cudaSuccess &&
+            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
+            n = v;
+        else
+            return 148;
+    }
+    return n;
+}
+
+// threads per CTA: real 15 consumer warps + 1 producer at <= 128 registers; complex holds twice the
+// registers per row (x and v are (re, im)), so 11 + 1 warps at <= 168 registers.
+template <bool CPLX, int NBW, int CPL>
+cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
+                          int64_t ldq, int align16, cudaStream_t st)
+{
+    using C = WinCfg<CPLX, NBW, CPL>;
+    constexpr int MAXT = CPLX ? 384 : 512;
+    auto kern = bt_window_kernel<CPLX, NBW, CPL, MAXT>;
+    static bool attr_done = false;
+    constexpr int NWMAX = MAXT / 32 - 1;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)C::smem_bytes(NWMAX));
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t units = (nev + C::CW - 1) / C::CW;
+    const int64_t nsm = sm_count();
+    const int64_t waves = (units + nsm * NWMAX - 1) / (nsm * NWMAX);
+    int64_t nw = (units + nsm * waves - 1) / (nsm * waves);
+    if (nw < 1) nw = 1;
+    if (nw > NWMAX) nw = NWMAX;
+    const int64_t grid = (units + nw - 1) / nw;
+    WinArgs a;
+    a.N = N;
+    a.nev = nev;
+    a.ldq = ldq;
+    a.hh_v = hh_v;
+    a.hh_tau = hh_tau;
+    a.q = q;
+    a.nw = (int)nw;
+    a.align16 = align16;
+    kern<<<(unsigned)grid, (unsigned)((nw + 1) * 32), C::smem_bytes((int)nw), st>>>(a);
+    return cudaGetLastError();
+}
+
+template <bool CPLX>
+int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+        void *stream)
+{
+    constexpr int EW = CPLX ? 2 : 1;
+    const int lg = lg_of(nbw);
+    if (N < 0) return -1;
+    if (lg < 0) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (N <= 1 || nev == 0) return 0;
+    if (!hh_v) return -4;
+    if (!hh_tau) return -5;
+    if (!q) return -6;
+    if (ldq < N) return -7;
+    if (((uintptr_t)hh_v & 15) != 0) return -4;
+    if (((uintptr_t)hh_tau & (8 * EW - 1)) != 0) return -5;
+    if (((uintptr_t)q & (8 * EW - 1)) != 0) return -6;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if (g_variant == 1) {
+        const unsigned grid = (unsigned)((nev + 127) / 128);
+        bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
+        e = cudaGetLastError();
+    } else {
+        const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
+        switch (nbw) {
+        case 32: e = launch_window<CPLX, 32, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 64: e = launch_window<CPLX, 64, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        default: e = launch_window<CPLX, 128, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        }
+    }
+    if (e != cudaSuccess) return (int)e;
+    g_last_launches = 1;
+    return 0;
+}
+
+// grow-only device scratch for the host-buffer entry point
+struct Scratch {
+    void *p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t n)
+    {
+        if (n <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr;
+        cap = 0;
+        cudaError_t e = cudaMalloc(&p, n);
+        if (e == cudaSuccess) cap = n;
+        return e;
+    }
+} g_sv, g_st, g_sq;
+
+}  // namespace
+
+extern "C" {
+
+int elpa2_trans_ev_tridi_to_band_d(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau,
+                                   double *q, int64_t ldq, void *stream)
+{
+    return run<false>(N, nbw, nev, hh_v, hh_tau, q, ldq, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_z(int64_t N, int nbw, int64_t nev, const void *hh_v, const void *hh_tau,
+                                   void *q, int64_t ldq, void *stream)
+{
+    return run<true>(N, nbw, nev, (const double *)hh_v, (const double *)hh_tau, (double *)q, ldq, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hh_v,
+                                      const void *hh_tau, void *q, int64_t ldq)
+{
+    const size_t esz = is_complex ? 16 : 8;
+    if (N < 0) return -1;
+    if (lg_of(nbw) < 0) return -2;
+    if (nev < 0) return -3;
+    if (N <= 1 || nev == 0) { g_last_launches = 0; return 0; }
+    if (!hh_v) return -4;
+    if (!hh_tau) return -5;
+    if (!q) return -6;
+    if (ldq < N) return -7;
+    std::lock_guard<std::mutex> lock(g_mu);
+    const size_t G = (size_t)elpa2_hh_count(N, nbw);
+    const size_t bv = G * nbw * esz, bt = G * esz, bq = (size_t)ldq * nev * esz;
+    cudaError_t e;
+    if ((e = g_sv.reserve(bv)) != cudaSuccess) return (int)e;
+    if ((e = g_st.reserve(bt)) != cudaSuccess) return (int)e;
+    if ((e = g_sq.reserve(bq)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sv.p, hh_v, bv, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_st.p, hh_tau, bt, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sq.p, q, bq, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    int rc = is_complex ? run<true>(N, nbw, nev, (const double *)g_sv.p, (const double *)g_st.p, (double *)g_sq.p, ldq, 0)
+                        : run<false>(N, nbw, nev, (const double *)g_sv.p, (const double *)g_st.p, (double *)g_sq.p, ldq, 0);
+    if (rc != 0) return rc;
+    if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
+    return 0;
+}
+
+int64_t elpa2_hh_count(int64_t N, int nbw)
+{
+    const int lg = lg_of(nbw);
+    if (lg < 0 || N < 2) return 0;
+    return hh_F(N - 1, lg);
+}
+
+int64_t elpa2_hh_offset(int64_t N, int nbw, int64_t s)
+{
+    const int lg = lg_of(nbw);
+    if (lg < 0 || N < 2 || s < 0 || s > N - 1) return -1;
+    return hh_off(N, lg, s);
+}
+
+int elpa2_hh_blocks(int64_t N, int nbw, int64_t s)
+{
+    const int lg = lg_of(nbw);
+    if (lg < 0 || N < 2 || s < 0 || s > N - 2) return 0;
+    return (int)((N - 1 - s + nbw - 1) >> lg);
+}
+
+int elpa2_bt_last_launch_count(void) { return g_last_launches; }
+
+int elpa2_bt_set_variant(int variant)
+{
+    if (variant < 0 || variant > 1) return -1;
+    const int old = g_variant;
+    g_variant = variant;
+    return old;
+}
+
+const char *elpa2_bt_version(void) { return "elpa2-bt-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"

@@ -1,0 +1,96 @@
+"""CPU-side checks of the C-ABI library: it loads, exports every symbol include/elpa2_bt.h
+declares, its integer layout helpers agree with the oracle's plain sums, and argument validation
+(which runs before any CUDA call) returns the documented codes.  No compute calls."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import oracle as orc
+from paper_2002_10991_b200 import binding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    binding.build()
+    return binding.lib()
+
+
+def test_header_symbols_exported(lib):
+    hdr = open(os.path.join(ROOT, "include", "elpa2_bt.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = set(re.findall(r"\b(elpa2_[a-z0-9_]+)\s*\(", hdr))
+    assert names == set(binding.EXPORTS)
+    for n in names:
+        assert getattr(lib, n) is not None
+    assert b"sm_100a" in lib.elpa2_bt_version()
+
+
+@pytest.mark.parametrize("N", [0, 1, 2, 3, 17, 33, 64, 65, 100, 129, 512, 1000])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_layout_helpers_match_oracle(lib, N, nbw):
+    assert binding.hh_count(N, nbw) == orc.hh_count(N, nbw)
+    for s in range(max(N - 1, 0)):
+        assert binding.hh_offset(N, nbw, s) == orc.hh_offset(N, nbw, s)
+        assert binding.hh_blocks(N, nbw, s) == orc.hh_blocks(N, nbw, s)
+    if N >= 2:
+        assert binding.hh_offset(N, nbw, N - 1) == orc.hh_count(N, nbw)
+        assert binding.hh_offset(N, nbw, N) == -1
+        assert binding.hh_blocks(N, nbw, N - 1) == 0
+
+
+def test_layout_full_size_counts(lib):
+    # G for the five configs
+    assert binding.hh_count(512, 32) == 4336
+    assert binding.hh_count(4096, 64) == 133056
+    assert binding.hh_count(8192, 64) == 528256
+    assert binding.hh_count(32768, 64) == 8404480
+    assert binding.hh_count(16384, 128) == 1056640
+    assert binding.hh_count(100, 48) == 0          # unsupported nbw
+
+
+def test_argument_validation_codes(lib):
+    buf = (ctypes.c_double * 64)()
+    p = ctypes.addressof(buf)
+    p16 = (p + 15) & ~15
+    call = binding.trans_ev_tridi_to_band_raw
+    for cplx in (False, True):
+        assert call(cplx, -1, 64, 4, p16, p16, p16, 8, 0) == -1
+        assert call(cplx, 8, 48, 4, p16, p16, p16, 8, 0) == -2
+        assert call(cplx, 8, 64, -4, p16, p16, p16, 8, 0) == -3
+        assert call(cplx, 8, 64, 4, 0, p16, p16, 8, 0) == -4
+        assert call(cplx, 8, 64, 4, p16 + 8, p16, p16, 8, 0) == -4
+        assert call(cplx, 8, 64, 4, p16, 0, p16, 8, 0) == -5
+        assert call(cplx, 8, 64, 4, p16, p16, 0, 8, 0) == -6
+        assert call(cplx, 8, 64, 4, p16, p16, p16 + 4, 8, 0) == -6
+        assert call(cplx, 8, 64, 4, p16, p16, p16, 7, 0) == -7
+        # no work: success without touching CUDA
+        assert call(cplx, 0, 64, 4, 0, 0, 0, 1, 0) == 0
+        assert call(cplx, 1, 64, 4, 0, 0, 0, 1, 0) == 0
+        assert call(cplx, 8, 64, 0, 0, 0, 0, 8, 0) == 0
+    assert lib.elpa2_trans_ev_tridi_to_band_host(0, 8, 40, 4, p16, p16, p16, 8) == -2
+    assert lib.elpa2_trans_ev_tridi_to_band_host(1, 8, 32, 4, p16, p16, p16, 4) == -7
+    assert binding.set_variant(7) == -1
+    assert binding.set_variant(0) in (0, 1)
+
+
+def test_no_gpu_fails_loudly(lib):
+    """Without a device the compute call must fail with a cudaError_t (> 0), never silently."""
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    buf = (ctypes.c_double * 4096)()
+    p16 = (ctypes.addressof(buf) + 15) & ~15
+    rc = binding.trans_ev_tridi_to_band_raw(False, 8, 32, 2, p16, p16, p16, 8, 0)
+    assert rc > 0
+
+
+def test_missing_library_raises(monkeypatch):
+    monkeypatch.setattr(binding, "_lib", None)
+    monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libelpa2_bt.so")
+    with pytest.raises(RuntimeError, match="no CPU fallback"):
+        binding.lib()

@@ -1,0 +1,146 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the
+same seeded inputs.  Tolerance from BASELINE.json north_star: max|dQ| <= 1e-11 * ||X||_max; a
+tighter diagnostic bound is asserted too: the two sides differ only in
+summation order, so the error must stay near 1e-15 * sqrt(N)-ish.
+"""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2002_10991_b200 import synth_inputs as si
+from gpu_util import run_gpu, oracle_apply
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-11
+
+
+def _tight(N):
+    return 2e-14 * max(1.0, (N / 64.0)) ** 0.5 * 8
+
+
+def _reflectors(N, nbw, seed, cplx):
+    ab = si.band_matrix(N, nbw, seed, cplx)
+    hh_v, hh_tau, d, e = orc.bulge_chase(ab, nbw)
+    return hh_v, hh_tau, d, e
+
+
+def _x(N, nev, seed, cplx):
+    rng = np.random.default_rng(seed)
+    x = rng.standard_normal((N, nev))
+    if cplx:
+        x = x + 1j * rng.standard_normal((N, nev))
+    return np.asfortranarray(x)
+
+
+def _check(N, nbw, nev, cplx, ldq=None, variant=0, seed=0):
+    hh_v, hh_tau, _, _ = _reflectors(N, nbw, 4000 + seed + N, cplx)
+    x = _x(N, nev, 17 + seed, cplx)
+    want = oracle_apply(N, nbw, hh_v, hh_tau, x)
+    got, pad = run_gpu(N, nbw, hh_v, hh_tau, x, ldq=ldq, variant=variant)
+    xmax = max(np.abs(x).max(initial=0.0), 1e-300)
+    err = np.abs(got - want).max(initial=0.0) / xmax
+    assert err <= TOL, (N, nbw, nev, cplx, err)
+    assert err <= _tight(N), (N, nbw, nev, cplx, err)
+    assert np.all(pad == 7.25)                       # rows N..ldq-1 untouched
+    return err
+
+
+# SURVEY.md section 4 tier T2: edge shapes around the window/tile/strip boundaries
+def _edge_N(nbw):
+    return [2, 3, 15, 16, 17, nbw - 1, nbw, nbw + 1, nbw + 2, 2 * nbw - 1, 2 * nbw + 1, 3 * nbw + 5]
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_edge_rows(nbw, cplx):
+    for N in _edge_N(nbw):
+        _check(N, nbw, 7, cplx)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+@pytest.mark.parametrize("nev", [1, 7, 33, 100])
+def test_edge_columns(nbw, nev, cplx):
+    _check(3 * nbw + 5, nbw, nev, cplx)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_ldq_padding_and_unaligned(nbw, cplx):
+    N = 2 * nbw + 9
+    _check(N, nbw, 19, cplx, ldq=N + 6)     # even ldq > N
+    _check(N, nbw, 19, cplx, ldq=N + 3)     # ldq*8 not 16-byte aligned -> 8-byte path (real)
+    _check(N + 1, nbw, 19, cplx, ldq=N + 1)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_nev_equals_N_square(cplx):
+    _check(200, 32, 200, cplx)
+    _check(333, 64, 333, cplx)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_many_warps_and_ctas(nbw, cplx):
+    # enough columns for several CTAs with several consumer warps each, ragged last strip
+    _check(5 * nbw + 3, nbw, 2500 + 13, cplx)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_simple_variant_matches_oracle(cplx):
+    _check(150, 32, 37, cplx, variant=1)
+    _check(300, 64, 21, cplx, variant=1)
+    _check(300, 128, 21, cplx, variant=1)
+
+
+def test_degenerate_no_work():
+    for N, nev in ((0, 5), (1, 5), (40, 0)):
+        x = np.zeros((N, nev), order="F")
+        got, _ = run_gpu(N, 32, np.zeros((0, 32)), np.zeros(0), x)
+        assert got.shape == (N, nev)
+
+
+def test_identity_reflectors_leave_q_bitwise():
+    N, nbw, nev = 200, 64, 50
+    G = orc.hh_count(N, nbw)
+    hh_v = np.zeros((G, nbw))
+    hh_v[:, 0] = 1.0
+    hh_tau = np.zeros(G)
+    x = _x(N, nev, 3, False)
+    got, _ = run_gpu(N, nbw, hh_v, hh_tau, x)
+    assert np.array_equal(got, x)
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+def test_host_entry_point(cplx):
+    from paper_2002_10991_b200 import binding
+
+    N, nbw, nev = 260, 64, 45
+    hh_v, hh_tau, _, _ = _reflectors(N, nbw, 77, cplx)
+    x = _x(N, nev, 5, cplx)
+    want = oracle_apply(N, nbw, hh_v, hh_tau, x)
+    y = np.array(x, order="F", copy=True)
+    binding.trans_ev_tridi_to_band_host(N, nbw, hh_v, hh_tau, y)
+    assert np.abs(y - want).max() <= TOL * np.abs(x).max()
+    assert binding.last_launch_count() == 1
+
+
+def test_launch_on_side_stream():
+    import torch
+
+    from paper_2002_10991_b200 import binding
+    from gpu_util import to_device_colmajor
+
+    N, nbw, nev = 300, 64, 64
+    hh_v, hh_tau, _, _ = _reflectors(N, nbw, 78, False)
+    x = _x(N, nev, 6, False)
+    want = oracle_apply(N, nbw, hh_v, hh_tau, x)
+    s = torch.cuda.Stream()
+    q = to_device_colmajor(x)
+    dv, dt = torch.from_numpy(hh_v).cuda(), torch.from_numpy(hh_tau).cuda()
+    torch.cuda.synchronize()
+    with torch.cuda.stream(s):
+        binding.trans_ev_tridi_to_band(N, nbw, dv, dt, q, stream=s)
+    s.synchronize()
+    assert np.abs(q.cpu().numpy() - want).max() <= TOL * np.abs(x).max()
