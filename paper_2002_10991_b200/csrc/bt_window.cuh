@@ -36,7 +36,11 @@ struct WinCfg {
     static constexpr int ESZ = 8 * EW;
     static constexpr int TSTRIDE = CPLX ? 17 : 18;   // tile column stride (elements): bank spread
     static constexpr int TILE_BYTES = CW * TSTRIDE * ESZ;
-    static constexpr int VBLK_BYTES = 16 * NBW * ESZ;
+    // v in shared memory: LPC groups of 16 rows, group stride padded by 16 bytes so that the LPC
+    // row lanes of a column (which read the same offset of different groups) hit different banks
+    static constexpr int GS = 16 + (CPLX ? 1 : 2);    // group stride (elements)
+    static constexpr int VS = LPC * GS;               // reflector stride (elements)
+    static constexpr int VBLK_BYTES = 16 * VS * ESZ;
     static constexpr int TAU_BYTES = 16 * ESZ;
     static constexpr int NS = (VBLK_BYTES > 16384) ? 3 : 4;   // ring stages
     static constexpr int OFF_TAU = NS * VBLK_BYTES;
@@ -124,7 +128,7 @@ __device__ __forceinline__ void tile_drain(const WinArgs &a, const double *tile,
 
 // ---- the kernel -------------------------------------------------------------------------------
 template <bool CPLX, int NBW, int CPL, int MAXT>
-__global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
+__global__ void __maxnreg__(65536 / MAXT / 8 * 8) bt_window_kernel(const WinArgs a)
 {
     using C = WinCfg<CPLX, NBW, CPL>;
     constexpr int EW = C::EW, LPC = C::LPC, NCG = C::NCG, NS = C::NS;
@@ -137,13 +141,12 @@ __global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int nw = a.nw;
     const int64_t units = (a.nev + C::CW - 1) / C::CW;            // warp-units in the whole call
-    const int64_t unit0 = (int64_t)blockIdx.x * nw;
-    int64_t nact = units - unit0;
-    nact = nact > nw ? nw : nact;                                   // active consumer warps here
+    const int64_t unit0 = units * blockIdx.x / gridDim.x;           // balanced split over CTAs
+    const int64_t nact = units * (blockIdx.x + 1) / gridDim.x - unit0;   // active consumer warps here
 
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
-            mbar_init(bar_full + 8 * i, 16);
+            mbar_init(bar_full + 8 * i, 32);
             mbar_init(bar_empty + 8 * i, (uint32_t)nact);
         }
         mbar_fence_init();
@@ -156,15 +159,17 @@ __global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
 
     if (warp == nw) {
         // ================= producer warp: stage reflectors in consumption order =================
-        if (lane >= 16) return;
-        const int u = lane;
+        // lane = u + 16*half: reflector u of the block; each half issues LPC/2 of its 16-row groups
+        const int u = lane & 15, half = lane >> 4;
+        constexpr int GPL = LPC / 2;                          // groups per lane
+        constexpr uint32_t GBYTES = 16 * C::ESZ;              // bytes per group
         const int64_t FN1 = hh_F(N - 1, C::LG);
         uint32_t it = 0;
         for (int64_t k = 0; k < K0; ++k) {
             const int64_t Bend = (1 + (k << C::LG)) >> 4;
             for (int64_t B = B0; B >= Bend; --B, ++it) {
                 const uint32_t st = it % NS, ph = (it / NS) & 1;
-                mbar_wait(bar_empty + 8 * st, ph ^ 1);
+                mbar_wait_backoff(bar_empty + 8 * st, ph ^ 1);
                 const int64_t r0 = (B << 4) + u;
                 const int64_t s = r0 - 1 - (k << C::LG);
                 const bool valid = (r0 <= N - 1) && (s >= 0);
@@ -175,12 +180,18 @@ __global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
                     tr = __ldg(a.hh_tau + g * EW);
                     if (CPLX) ti = __ldg(a.hh_tau + g * EW + 1);
                 }
-                ring_tau[(st * 16 + u) * EW] = tr;
-                if (CPLX) ring_tau[(st * 16 + u) * EW + 1] = ti;
+                if (half == 0) {
+                    ring_tau[(st * 16 + u) * EW] = tr;
+                    if (CPLX) ring_tau[(st * 16 + u) * EW + 1] = ti;
+                }
                 if (valid && (tr != 0.0 || ti != 0.0)) {
-                    mbar_arrive_expect_tx(bar_full + 8 * st, NBW * C::ESZ);
-                    bulk_g2s(smem_u32(ring_v + ((size_t)st * 16 + u) * NBW * EW), a.hh_v + g * NBW * EW,
-                             NBW * C::ESZ, bar_full + 8 * st);
+                    mbar_arrive_expect_tx(bar_full + 8 * st, GPL * GBYTES);
+#pragma unroll
+                    for (int gg = 0; gg < GPL; ++gg) {
+                        const int grp = half * GPL + gg;
+                        bulk_g2s(smem_u32(ring_v + ((size_t)(st * 16 + u) * C::VS + grp * C::GS) * EW),
+                                 a.hh_v + (g * NBW + grp * 16) * EW, GBYTES, bar_full + 8 * st);
+                    }
                 } else {
                     mbar_arrive(bar_full + 8 * st);
                 }
@@ -213,10 +224,10 @@ __global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
             cp_async_commit();
             const uint32_t st = it % NS, ph = (it / NS) & 1;
             mbar_wait(bar_full + 8 * st, ph);
-            const double *vb = ring_v + (size_t)st * 16 * NBW * EW;
+            const double *vb = ring_v + (size_t)st * 16 * C::VS * EW;
             const double *tb = ring_tau + st * 16 * EW;
-            const double *v0 = vb + (((l - (int)B) & (LPC - 1)) * 16) * EW;       // slots i >= u
-            const double *v1 = vb + (((l - (int)B - 1) & (LPC - 1)) * 16) * EW;   // slots i <  u
+            const double *v0 = vb + (((l - (int)B) & (LPC - 1)) * C::GS) * EW;       // slots i >= u
+            const double *v1 = vb + (((l - (int)B - 1) & (LPC - 1)) * C::GS) * EW;   // slots i <  u
             const bool act = (l == ((int)B & (LPC - 1)));
             double *tl = tiles + (B & 1) * (C::TILE_BYTES / 8) + cg * C::TSTRIDE * EW;
 #pragma unroll
@@ -245,8 +256,8 @@ __global__ void __launch_bounds__(MAXT, 1) bt_window_kernel(const WinArgs a)
                     double vv[16 * EW];
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
-                        const double *src = (i >= u) ? v0 + (u * NBW + (i - u)) * EW
-                                                     : v1 + (u * NBW + (16 + i - u)) * EW;
+                        const double *src = (i >= u) ? v0 + (u * C::VS + (i - u)) * EW
+                                                     : v1 + (u * C::VS + (16 + i - u)) * EW;
                         if (CPLX) {
                             const double2 t2 = *reinterpret_cast<const double2 *>(src);
                             vv[2 * i] = t2.x;

@@ -34,14 +34,14 @@ int sm_count()
     return n;
 }
 
-// threads per CTA: real 15 consumer warps + 1 producer at <= 128 registers; complex holds twice the
-// registers per row (x and v are (re, im)), so 11 + 1 warps at <= 168 registers.
+// threads per CTA: 8 consumer warps + 1 producer warp (2 consumer warps per SM sub-partition), up
+// to 224 registers per thread: the window (CPL columns x 16 rows per lane) takes 128 of them.
 template <bool CPLX, int NBW, int CPL>
 cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
                           int64_t ldq, int align16, cudaStream_t st)
 {
     using C = WinCfg<CPLX, NBW, CPL>;
-    constexpr int MAXT = CPLX ? 384 : 512;
+    constexpr int MAXT = 288;
     auto kern = bt_window_kernel<CPLX, NBW, CPL, MAXT>;
     static bool attr_done = false;
     constexpr int NWMAX = MAXT / 32 - 1;
@@ -54,10 +54,9 @@ cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const doub
     const int64_t units = (nev + C::CW - 1) / C::CW;
     const int64_t nsm = sm_count();
     const int64_t waves = (units + nsm * NWMAX - 1) / (nsm * NWMAX);
-    int64_t nw = (units + nsm * waves - 1) / (nsm * waves);
-    if (nw < 1) nw = 1;
-    if (nw > NWMAX) nw = NWMAX;
-    const int64_t grid = (units + nw - 1) / nw;
+    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
+    if (grid > units) grid = units;                   // ... unless there are fewer warp-units
+    const int64_t nw = (units + grid - 1) / grid;     // the kernel splits the units evenly over CTAs
     WinArgs a;
     a.N = N;
     a.nev = nev;
@@ -98,9 +97,9 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
     } else {
         const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
         switch (nbw) {
-        case 32: e = launch_window<CPLX, 32, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        case 64: e = launch_window<CPLX, 64, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        default: e = launch_window<CPLX, 128, CPLX ? 1 : 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 32: e = launch_window<CPLX, 32, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 64: e = launch_window<CPLX, 64, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        default: e = launch_window<CPLX, 128, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
         }
     }
     if (e != cudaSuccess) return (int)e;
