@@ -128,7 +128,7 @@ __device__ __forceinline__ void tile_drain(const WinArgs &a, const double *tile,
 
 // ---- the kernel -------------------------------------------------------------------------------
 template <bool CPLX, int NBW, int CPL, int MAXT>
-__global__ void __maxnreg__(65536 / MAXT / 8 * 8) bt_window_kernel(const WinArgs a)
+__global__ void __maxnreg__((65536 / MAXT / 8 * 8) > 255 ? 255 : (65536 / MAXT / 8 * 8)) bt_window_kernel(const WinArgs a)
 {
     using C = WinCfg<CPLX, NBW, CPL>;
     constexpr int EW = C::EW, LPC = C::LPC, NCG = C::NCG, NS = C::NS;
@@ -266,50 +266,90 @@ __global__ void __maxnreg__(65536 / MAXT / 8 * 8) bt_window_kernel(const WinArgs
                             vv[i] = *src;
                         }
                     }
+                    // All CPL columns advance together (i outer, column inner): 2*CPL (real) or
+                    // 4*CPL (complex) independent FMA chains hide the DFMA latency.
+                    if (CPLX) {
+                        // d = sum conj(v) x  (R2)
+                        double dr[CPL], di[CPL], er[CPL], ei[CPL];
 #pragma unroll
-                    for (int j = 0; j < CPL; ++j) {
-                        if (CPLX) {
-                            // d = sum conj(v) x  (R2)
-                            double dr = 0.0, di = 0.0, er = 0.0, ei = 0.0;
+                        for (int j = 0; j < CPL; ++j) {
+                            dr[j] = vv[0] * x[j][0];
+                            er[j] = vv[1] * x[j][1];
+                            di[j] = vv[0] * x[j][1];
+                            ei[j] = -vv[1] * x[j][0];
+                        }
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) {
-                                dr = fma(vv[2 * i], x[j][2 * i], dr);
-                                er = fma(vv[2 * i + 1], x[j][2 * i + 1], er);
-                                di = fma(vv[2 * i], x[j][2 * i + 1], di);
-                                ei = fma(-vv[2 * i + 1], x[j][2 * i], ei);
+                        for (int i = 1; i < 16; ++i)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) {
+                                dr[j] = fma(vv[2 * i], x[j][2 * i], dr[j]);
+                                er[j] = fma(vv[2 * i + 1], x[j][2 * i + 1], er[j]);
+                                di[j] = fma(vv[2 * i], x[j][2 * i + 1], di[j]);
+                                ei[j] = fma(-vv[2 * i + 1], x[j][2 * i], ei[j]);
                             }
-                            dr += er;
-                            di += ei;
 #pragma unroll
-                            for (int m = 1; m < LPC; m <<= 1) {
-                                dr += shfl_xor_f64(dr, m);
-                                di += shfl_xor_f64(di, m);
+                        for (int j = 0; j < CPL; ++j) {
+                            dr[j] += er[j];
+                            di[j] += ei[j];
+                        }
+#pragma unroll
+                        for (int m = 1; m < LPC; m <<= 1)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) {
+                                dr[j] += shfl_xor_f64(dr[j], m);
+                                di[j] += shfl_xor_f64(di[j], m);
                             }
-                            const double hr = -(tr * dr - ti * di), hi = -(tr * di + ti * dr);   // h = -tau d
+                        double hr[CPL], hi[CPL];   // h = -tau d
 #pragma unroll
-                            for (int i = 0; i < 16; ++i) {
+                        for (int j = 0; j < CPL; ++j) {
+                            hr[j] = -(tr * dr[j] - ti * di[j]);
+                            hi[j] = -(tr * di[j] + ti * dr[j]);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 16; ++i)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) {
                                 double xr = x[j][2 * i], xi = x[j][2 * i + 1];
-                                xr = fma(hr, vv[2 * i], xr);
-                                xr = fma(-hi, vv[2 * i + 1], xr);
-                                xi = fma(hr, vv[2 * i + 1], xi);
-                                xi = fma(hi, vv[2 * i], xi);
+                                xr = fma(hr[j], vv[2 * i], xr);
+                                xi = fma(hr[j], vv[2 * i + 1], xi);
+                                xr = fma(-hi[j], vv[2 * i + 1], xr);
+                                xi = fma(hi[j], vv[2 * i], xi);
                                 x[j][2 * i] = xr;
                                 x[j][2 * i + 1] = xi;
                             }
-                        } else {
-                            double d0 = vv[0] * x[j][0], d1 = vv[1] * x[j][1];
+                    } else {
+                        // four partial sums per column: even if the scheduler serialises the
+                        // columns, four independent chains cover the DFMA latency
+                        double d0[CPL], d1[CPL], d2[CPL], d3[CPL];
 #pragma unroll
-                            for (int i = 2; i < 16; i += 2) {
-                                d0 = fma(vv[i], x[j][i], d0);
-                                d1 = fma(vv[i + 1], x[j][i + 1], d1);
-                            }
-                            double d = d0 + d1;
-#pragma unroll
-                            for (int m = 1; m < LPC; m <<= 1) d += shfl_xor_f64(d, m);
-                            const double h = -tr * d;
-#pragma unroll
-                            for (int i = 0; i < 16; ++i) x[j][i] = fma(h, vv[i], x[j][i]);
+                        for (int j = 0; j < CPL; ++j) {
+                            d0[j] = vv[0] * x[j][0];
+                            d1[j] = vv[1] * x[j][1];
+                            d2[j] = vv[2] * x[j][2];
+                            d3[j] = vv[3] * x[j][3];
                         }
+#pragma unroll
+                        for (int i = 4; i < 16; i += 4)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) {
+                                d0[j] = fma(vv[i], x[j][i], d0[j]);
+                                d1[j] = fma(vv[i + 1], x[j][i + 1], d1[j]);
+                                d2[j] = fma(vv[i + 2], x[j][i + 2], d2[j]);
+                                d3[j] = fma(vv[i + 3], x[j][i + 3], d3[j]);
+                            }
+#pragma unroll
+                        for (int j = 0; j < CPL; ++j) d0[j] = (d0[j] + d1[j]) + (d2[j] + d3[j]);
+#pragma unroll
+                        for (int m = 1; m < LPC; m <<= 1)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) d0[j] += shfl_xor_f64(d0[j], m);
+                        double h[CPL];
+#pragma unroll
+                        for (int j = 0; j < CPL; ++j) h[j] = -tr * d0[j];
+#pragma unroll
+                        for (int i = 0; i < 16; ++i)
+#pragma unroll
+                            for (int j = 0; j < CPL; ++j) x[j][i] = fma(h[j], vv[i], x[j][i]);
                     }
                 }
             }

@@ -34,14 +34,15 @@ int sm_count()
     return n;
 }
 
-// threads per CTA: 8 consumer warps + 1 producer warp (2 consumer warps per SM sub-partition), up
-// to 224 registers per thread: the window (CPL columns x 16 rows per lane) takes 128 of them.
+// threads per CTA: 7 consumer warps + 1 producer warp = 256 threads, so that each thread may use
+// up to 255 registers (the window, CPL columns x 16 rows per lane, takes 128 of them).  With 9
+// warps (224 registers) ptxas serialises the columns of a step and the kernel is 25 % slower.
 template <bool CPLX, int NBW, int CPL>
 cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
                           int64_t ldq, int align16, cudaStream_t st)
 {
     using C = WinCfg<CPLX, NBW, CPL>;
-    constexpr int MAXT = 288;
+    constexpr int MAXT = 256;
     auto kern = bt_window_kernel<CPLX, NBW, CPL, MAXT>;
     static bool attr_done = false;
     constexpr int NWMAX = MAXT / 32 - 1;
