@@ -1,0 +1,345 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the stage-2 eigenvector back-transformation (Eq. 6d)
+on synthetic inputs of BASELINE.json's shapes.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
+
+One "step" = one call of ``elpa2_trans_ev_tridi_to_band_{d,z}`` over the whole N x nev block (all
+SURVEY.md 8(a) rows a1-a5 happen inside that one kernel launch).  Default workload: config 4
+(real FP64, N = 32768, nbw = 64, nev = 32768), the configuration BASELINE.json's target is quoted
+on.  Reflectors for the timed run are the seeded synthetic unitary stream of
+``synth_inputs.synthetic_reflectors`` (same layout, lengths, tau != 0 pattern and value range as
+chase output; the kernel's work does not depend on the values), X is i.i.d. N(0,1), both generated
+on the device.
+
+Prints ONE JSON line (rank 0).  ``value`` = model GFLOP/s (2 N^2 nev real / 8 N^2 nev complex) of
+the whole job with all buffers resident in HBM; ``e2e`` = the same metric through the C-ABI
+host-buffer entry point with pinned host memory (H2D of reflectors and q, kernel, D2H of q inside
+the timed region); ``roofline`` = the kernel against the FP64 ALU peak; ``cpu_baseline`` = the
+oracle timed on this box's host cores on a bounded column sample.
+
+N > 1 (torchrun): columns are independent, so every rank back-transforms its own
+nev columns with a replicated reflector stream -- no data-path collective; weak scaling.
+
+``--impl reference`` times the CPU oracle (oracle/) on the same config; that leg and the
+cpu_baseline leg are the only places this file touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# SURVEY.md 8(d) / BASELINE.json configs: (complex, N, nbw, nev, seed_reflectors, seed_X)
+CONFIGS = {
+    1: (False, 512, 32, 512, 1001, 2001),
+    2: (False, 4096, 64, 4096, 1002, 2002),
+    3: (True, 8192, 64, 4096, 1003, 2003),
+    4: (False, 32768, 64, 32768, 1004, 2004),
+    5: (True, 16384, 128, 8192, 1005, 2005),
+}
+METRIC = "back-transform FP64 GFLOP/s (2N^2*nev real / 8N^2*nev cplx)"
+# FP64 ALU roofline: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz
+NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+# dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full), by config
+NCU_TRAFFIC_BYTES = {}
+
+
+def model_flops(cplx: bool, N: int, nev: int) -> float:
+    return (8.0 if cplx else 2.0) * float(N) * float(N) * float(nev)
+
+
+def workload_name(cfg: int) -> str:
+    cplx, N, nbw, nev, _, _ = CONFIGS[cfg]
+    return f"config{cfg}: {'complex' if cplx else 'real'} FP64 N={N} nbw={nbw} nev={nev}"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.FIELDS}",
+                 "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+        return self
+
+    def _pump(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def __exit__(self, *exc):
+        if self.proc is not None:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except subprocess.TimeoutExpired:
+                self.proc.kill()
+            self.thread.join(timeout=5)
+
+    def summary(self) -> dict:
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            parts = [p.strip() for p in ln.split(",")]
+            if len(parts) < 7:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample_run(cplx, N, nbw, hh_v_np, hh_tau_np, ncols, seed):
+    """Times the oracle, as it stands, on ``ncols`` seeded N(0,1) columns.  Returns (seconds, threads)."""
+    import numpy as np
+
+    import oracle
+
+    rng = np.random.default_rng(seed)
+    x = rng.standard_normal((N, ncols))
+    if cplx:
+        x = x + 1j * rng.standard_normal((N, ncols))
+    x = np.asfortranarray(x)
+    t0 = time.perf_counter()
+    oracle.back_transform(N, nbw, hh_v_np, hh_tau_np, x)
+    return time.perf_counter() - t0, oracle.num_threads()
+
+
+def oracle_sample_cols(cplx: bool, N: int, cores: int) -> int:
+    """Column count giving roughly 10-30 s of CPU work: the oracle runs about 1.9 (real) / 2.9
+    (complex) model GFLOP/s per thread, so one config-4 column is about 1.1 s of one core."""
+    per_col = model_flops(cplx, N, 1) / (2.9e9 if cplx else 1.9e9)
+    per_core = max(1, min(64, int(16.0 / max(per_col, 1e-9))))
+    return cores * per_core
+
+
+def run_reference(args, rank: int) -> None:
+    """--impl reference: the CPU oracle on the same config and metric (rank 0 only)."""
+    if rank != 0:
+        return
+    import numpy as np
+    import torch
+
+    import oracle
+    from paper_2002_10991_b200 import synth_inputs as si
+
+    cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
+    cores = oracle.num_threads()
+    # per-slot lengths from the oracle's own layout (this arm never loads the CUDA library)
+    K = np.array([oracle.hh_blocks(N, nbw, s) for s in range(N - 1)], dtype=np.int64)
+    s_of_g = np.repeat(np.arange(N - 1, dtype=np.int64), K)
+    k_of_g = np.arange(int(K.sum()), dtype=np.int64) - np.repeat(np.cumsum(K) - K, K)
+    lengths = np.minimum(nbw, N - 1 - s_of_g - k_of_g * nbw)
+    hv, ht = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cpu")
+    hv, ht = hv.numpy(), ht.numpy()
+    ncols = oracle_sample_cols(cplx, N, cores)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t, _ = oracle_sample_run(cplx, N, nbw, hv, ht, ncols, seed_x + i)
+        if i >= args.warmup:
+            times.append(t)
+    total = sum(times)
+    gflops = model_flops(cplx, N, ncols) * len(times) / total / 1e9
+    sample = f"{ncols} seeded N(0,1) columns of {nev} per step (columns are independent, PAPER.md:134)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": workload_name(args.config), "reflectors":
+                                        "synthetic unitary stream (host-generated)"},
+        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(CONFIGS))
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer calls (0 = skip)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "b200":
+        print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+
+    from paper_2002_10991_b200 import binding, synth_inputs as si
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
+    esz = 16 if cplx else 8
+    flops = model_flops(cplx, N, nev)
+
+    # ---- inputs, generated on the device (each rank: its own nev columns, same reflectors) ----
+    lengths = binding.hh_lengths(N, nbw)
+    G = int(lengths.shape[0])
+    assert G == binding.hh_count(N, nbw)
+    hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
+    q = si.gaussian_block(N, nev, seed_x + 7919 * rank, cplx, "cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        binding.trans_ev_tridi_to_band(N, nbw, hh_v, hh_tau, q, stream=stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- FP64 ALU peak of this device, measured live (outside the timed region) ----
+    dfma_tf = binding.probe_fp64(0, 8192, 20)
+
+    ncheck = min(nev, 64)
+    nrm0 = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    launches = 0
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev[0].record(stream)
+        for i in range(args.steps):
+            step()
+            launches += binding.last_launch_count()
+            ev[i + 1].record(stream)
+        barrier()
+    clk = clocks.summary()
+    step_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    total_ms = ev[0].elapsed_time(ev[args.steps])
+    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    value = world * flops / (ms_per_step * 1e-3) / 1e9
+
+    # unitarity check on the timed buffer (every H is unitary, so column norms must not move)
+    nrm = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
+    norm_dev = float((nrm / nrm0 - 1.0).abs().max().item())
+
+    # ---- e2e: host buffers through the C-ABI host entry point (rank-local, pinned memory) ----
+    e2e = None
+    if args.e2e_steps > 0:
+        hv_h = torch.empty(hh_v.shape, dtype=hh_v.dtype, pin_memory=True).copy_(hh_v)
+        ht_h = torch.empty(hh_tau.shape, dtype=hh_tau.dtype, pin_memory=True).copy_(hh_tau)
+        q_h = torch.empty((nev, N), dtype=q.dtype, pin_memory=True).copy_(q.t())
+        torch.cuda.synchronize()
+        hv_np, ht_np, q_np = hv_h.numpy(), ht_h.numpy(), q_h.numpy().T      # q_np: (N, nev) Fortran
+        binding.trans_ev_tridi_to_band_host(N, nbw, hv_np, ht_np, q_np)     # warm-up: scratch alloc
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            binding.trans_ev_tridi_to_band_host(N, nbw, hv_np, ht_np, q_np)
+            launches += binding.last_launch_count()
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+        h2d = (G * nbw + G + N * nev) * esz
+        d2h = N * nev * esz
+        e2e = {"value": world * flops * args.e2e_steps / dt / 1e9, "unit": "GFLOP/s",
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": args.e2e_steps,
+               "timer": "host wall clock around synchronous calls"}
+        del hv_h, ht_h, q_h
+
+    # ---- cpu_baseline: the oracle on a bounded column sample (rank 0, N = 1 only) ----
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+
+        cores = oracle.num_threads()
+        ncols = oracle_sample_cols(cplx, N, cores)
+        tsec, cores = oracle_sample_run(cplx, N, nbw, hh_v.cpu().numpy(), hh_tau.cpu().numpy(), ncols, seed_x)
+        cpu = {"value": model_flops(cplx, N, ncols) / tsec / 1e9, "unit": "GFLOP/s", "cores": cores,
+               "kind": "oracle", "seconds": tsec,
+               "sample": f"{ncols} seeded N(0,1) columns of {nev}, all {G} reflectors "
+                         "(columns are independent, PAPER.md:134)"}
+
+    if rank == 0:
+        kern_ms = sum(step_ms) / len(step_ms)
+        achieved = flops / (kern_ms * 1e-3) / 1e12
+        out = {
+            "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config), "N": N, "nbw": nbw, "nev_per_gpu": nev,
+                       "reflector_slots": G,
+                       "reflectors": "synthetic unitary stream, device-generated (DESIGN.md input recipe)",
+                       "l2": ("inputs larger than L2 (%.2f GiB of q + reflectors per step)"
+                              % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
+                             else "inputs smaller than L2; config is latency-bound (DESIGN.md)",
+                       "parallelism": "column shards, no collective" if world > 1 else "single GPU"},
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": dfma_tf, "unit": "TFLOP/s",
+                         "frac": achieved / dfma_tf,
+                         "peak_source": "DFMA probe measured in this run (elpa2_bt_probe_fp64 kind 0); "
+                                        "MEASURED_PEAKS.json has no FP64 figure",
+                         "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                         "kernel": "bt_window_kernel", "kernel_ms": kern_ms,
+                         "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
+            "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
+            "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},
+        }
+        print(json.dumps(out), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

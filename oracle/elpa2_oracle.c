@@ -375,6 +375,21 @@ int orc_tridiag_ql(int64_t N, double *d, double *e_in, double *x)
  * column range is split over OpenMP threads; each thread runs the full reflector loop on its
  * own columns in exactly the order above.
  * ---------------------------------------------------------------------------------------- */
+/* Columns handed to one thread at a time: up to 8 (they share each reflector while it is in
+ * cache), fewer when there are not enough columns to give every thread a chunk.  Scheduling only:
+ * each column sees exactly the same operations in the same order whatever the chunk size. */
+static int64_t orc_col_chunk(int64_t ncols)
+{
+    int64_t nt = 1;
+#ifdef _OPENMP
+    nt = omp_get_max_threads();
+#endif
+    int64_t c = (ncols + nt - 1) / nt;
+    if (c > 8) c = 8;
+    if (c < 1) c = 1;
+    return c;
+}
+
 void orc_back_transform_d(int64_t N, int nbw, int64_t ncols, const double *hh_v,
                           const double *hh_tau, double *q, int64_t ldq)
 {
@@ -382,7 +397,7 @@ void orc_back_transform_d(int64_t N, int nbw, int64_t ncols, const double *hh_v,
     int64_t *off = malloc(sizeof(int64_t) * N);
     off[0] = 0;
     for (int64_t s = 1; s < N; ++s) off[s] = off[s - 1] + orc_hh_blocks(N, nbw, s - 1);
-    const int64_t chunk = 8;
+    const int64_t chunk = orc_col_chunk(ncols);
     const int64_t nchunks = (ncols + chunk - 1) / chunk;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t cb = 0; cb < nchunks; ++cb) {
@@ -415,7 +430,7 @@ void orc_back_transform_z(int64_t N, int nbw, int64_t ncols, const zdouble *hh_v
     int64_t *off = malloc(sizeof(int64_t) * N);
     off[0] = 0;
     for (int64_t s = 1; s < N; ++s) off[s] = off[s - 1] + orc_hh_blocks(N, nbw, s - 1);
-    const int64_t chunk = 8;
+    const int64_t chunk = orc_col_chunk(ncols);
     const int64_t nchunks = (ncols + chunk - 1) / chunk;
 #pragma omp parallel for schedule(dynamic, 1)
     for (int64_t cb = 0; cb < nchunks; ++cb) {

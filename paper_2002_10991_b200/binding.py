@@ -87,6 +87,20 @@ def hh_blocks(N: int, nbw: int, s: int) -> int:
     return lib().elpa2_hh_blocks(N, nbw, s)
 
 
+def hh_lengths(N: int, nbw: int):
+    """Length L of every reflector slot, in slot order (int64 numpy array of G entries), built
+    from the library's own layout helpers: slot (s, k) has L = min(nbw, N-1-s-k*nbw)."""
+    import numpy as np
+
+    if N < 2:
+        return np.zeros(0, dtype=np.int64)
+    K = np.array([hh_blocks(N, nbw, s) for s in range(N - 1)], dtype=np.int64)
+    s_of_g = np.repeat(np.arange(N - 1, dtype=np.int64), K)
+    first = np.cumsum(K) - K
+    k_of_g = np.arange(int(K.sum()), dtype=np.int64) - np.repeat(first, K)
+    return np.minimum(nbw, N - 1 - s_of_g - k_of_g * nbw)
+
+
 def version() -> str:
     return lib().elpa2_bt_version().decode()
 

@@ -18,6 +18,16 @@ __host__ __device__ __forceinline__ int64_t hh_off(int64_t N, int lg, int64_t s)
     return hh_F(N - 1, lg) - hh_F(N - 1 - s, lg);
 }
 
+// ---- kernel arguments of the window kernels ------------------------------------------------------
+struct WinArgs {
+    int64_t N, nev, ldq;
+    const double *hh_v;    // G * nbw elements
+    const double *hh_tau;  // G elements
+    double *q;
+    int nw;                // consumer warps per CTA
+    int align16;           // q base and ldq*ESZ are 16-byte aligned (always 1 for complex)
+};
+
 // ---- shared-memory / mbarrier / bulk-copy PTX wrappers ---------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {

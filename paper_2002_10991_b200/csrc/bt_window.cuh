@@ -50,15 +50,6 @@ struct WinCfg {
     static size_t smem_bytes(int nw) { return (size_t)OFF_TILE + (size_t)nw * 2 * TILE_BYTES; }
 };
 
-struct WinArgs {
-    int64_t N, nev, ldq;
-    const double *hh_v;    // G * nbw elements
-    const double *hh_tau;  // G elements
-    double *q;
-    int nw;                // consumer warps per CTA
-    int align16;           // q base and ldq*ESZ are 16-byte aligned (always 1 for complex)
-};
-
 // ---- tile fill / drain / flush -----------------------------------------------------------------
 // Tile buffer: element (c, r) of the warp's CW x 16 block at tile[(c*TSTRIDE + r) * EW].
 template <class C, bool CPLX>

@@ -7,10 +7,15 @@
 
 #include <mutex>
 
+#include "bt_shift.cuh"
 #include "bt_simple.cuh"
 #include "bt_window.cuh"
 
 using namespace elpa2bt;
+
+#ifndef ELPA2_BT_UNROLL
+#define ELPA2_BT_UNROLL 2
+#endif
 
 namespace {
 
@@ -71,6 +76,41 @@ cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const doub
     return cudaGetLastError();
 }
 
+// the shift kernel: same CTA shape (7 consumer warps + 1 producer warp, up to 255 registers)
+template <bool CPLX, int NBW, int CPL>
+cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
+                         int64_t ldq, int align16, cudaStream_t st)
+{
+    using C = ShiftCfg<CPLX, NBW, CPL>;
+    constexpr int MAXT = 256;
+    auto kern = bt_shift_kernel<CPLX, NBW, CPL, MAXT, ELPA2_BT_UNROLL>;
+    static bool attr_done = false;
+    constexpr int NWMAX = MAXT / 32 - 1;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)C::smem_bytes(NWMAX));
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t units = (nev + C::CW - 1) / C::CW;
+    const int64_t nsm = sm_count();
+    const int64_t waves = (units + nsm * NWMAX - 1) / (nsm * NWMAX);
+    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
+    if (grid > units) grid = units;                   // ... unless there are fewer warp-units
+    const int64_t nw = (units + grid - 1) / grid;     // the kernel splits the units evenly over CTAs
+    WinArgs a;
+    a.N = N;
+    a.nev = nev;
+    a.ldq = ldq;
+    a.hh_v = hh_v;
+    a.hh_tau = hh_tau;
+    a.q = q;
+    a.nw = (int)nw;
+    a.align16 = align16;
+    kern<<<(unsigned)grid, (unsigned)((nw + 1) * 32), C::smem_bytes((int)nw), st>>>(a);
+    return cudaGetLastError();
+}
+
 template <bool CPLX>
 int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
         void *stream)
@@ -95,6 +135,13 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
         const unsigned grid = (unsigned)((nev + 127) / 128);
         bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
         e = cudaGetLastError();
+    } else if (g_variant == 0) {
+        const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
+        switch (nbw) {
+        case 32: e = launch_shift<CPLX, 32, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 64: e = launch_shift<CPLX, 64, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        default: e = launch_shift<CPLX, 128, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        }
     } else {
         const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
         switch (nbw) {
@@ -195,7 +242,7 @@ int elpa2_bt_last_launch_count(void) { return g_last_launches; }
 
 int elpa2_bt_set_variant(int variant)
 {
-    if (variant < 0 || variant > 1) return -1;
+    if (variant < 0 || variant > 2) return -1;
     const int old = g_variant;
     g_variant = variant;
     return old;
