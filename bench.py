@@ -59,6 +59,8 @@ def model_flops(cplx: bool, N: int, nev: int) -> float:
 
 def workload_name(cfg: int) -> str:
     cplx, N, nbw, nev, _, _ = CONFIGS[cfg]
+    if cfg == 0:
+        return f"custom (--shape): {'complex' if cplx else 'real'} FP64 N={N} nbw={nbw} nev={nev}"
     return f"config{cfg}: {'complex' if cplx else 'real'} FP64 N={N} nbw={nbw} nev={nev}"
 
 
@@ -194,9 +196,16 @@ def main() -> None:
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer calls (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",
+                    help="profiling aid: replace the chosen config's shape (named 'custom' in the output)")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "b200":
         print(f"note: --warmup {args.warmup} < 3 breaks the timing rules", file=sys.stderr)
+
+    if args.shape:
+        t, n_, b_, e_ = args.shape.split(",")
+        CONFIGS[0] = (t == "z", int(n_), int(b_), int(e_), 1000, 2000)
+        args.config = 0
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -331,7 +340,7 @@ def main() -> None:
                          "peak_source": "DFMA probe measured in this run (elpa2_bt_probe_fp64 kind 0); "
                                         "MEASURED_PEAKS.json has no FP64 figure",
                          "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                         "kernel": "bt_window_kernel", "kernel_ms": kern_ms,
+                         "kernel": "bt_shift_kernel", "kernel_ms": kern_ms,
                          "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},
