@@ -1,0 +1,436 @@
+// bt_wy.cuh -- compact-WY back-transformation on the FP64 tensor cores (DMMA m8n8k4), real FP64,
+// sm_100a.  What it computes: include/elpa2_bt.h (Eq. 6d, Eq. 8).
+//
+// M = 8 consecutive reflectors of a chain (first rows r0 = 8b+7, 8b+6, .., 8b: applied in that
+// order) are aggregated (R6; PAPER.md:54, :101 cite the technique):
+//      H_7 .. H_1 H_0 = I - V T V^T,   T lower triangular, T[j][j] = tau_j,
+//      T[j][:j] = -tau_j (v_j^T V[:, :j]) T[:j, :j],
+// where V is the W x 8 matrix (W = nbw + 8 window rows 8b .. 8b+W-1) whose column i holds v_i at
+// row offset 7 - i.  Per block and per slab of 8 columns the window x (W x 8) is updated by
+//      D^T = x^T V        (8 cols x 8 refl, K = W rows)       W/4  DMMAs
+//      E^T = D^T (-T)^T   (8 cols x 8 refl, K = 8)            2    DMMAs
+//      x^T += E^T V^T     (8 cols x W rows, K = 8)            W/4  DMMAs
+// i.e. (nbw/2 + 6) DMMAs for the nbw/2 DMMA-equivalents of useful work (4 L flops per reflector
+// and column): 84 % at nbw = 64.  All three products keep "column of q" on the M index of the
+// fragment (lane / 4) and permute the K index so that the C fragment of one product IS the A
+// fragment of the next: no shuffles, no shared-memory round trip for x, D or E.
+//
+//  * x^T fragment: lane (gq = lane/4, r = lane%4) holds rows 8t + 2r + {0,1} of column gq for
+//    every 8-row tile t of the window: NT = W/8 register pairs per slab.  This is the C layout of
+//    the update (M = column, N = row in tile) and, read as "k-slot r of k-chunk (t,e) is row
+//    8t + 2r + e", the A layout of the dot product.
+//  * The window moves up by 8 rows = one tile per block: the update of tile t writes its result
+//    into the registers of tile t+1 (D != C in the DMMA), tile NT-1 retires to global memory
+//    (16 bytes per lane, 64 contiguous bytes per column), tile 0 is loaded for the next block.
+//  * V is staged in shared memory twice per block -- VA[i][w] (B fragments of the dot product) and
+//    VB[w][i] (B fragments of the update) -- by 8-byte cp.async straight from hh_v (the skew 7 - i
+//    breaks the 16-byte alignment bulk copies need); -T comes from a scratch array filled by
+//    wy_prepass_kernel (one warp per block: Gram matrix V^T V by DMMA, then the recurrence).
+//  * 8 warps per CTA (2 per SM sub-partition, 255 registers), no producer warp: the warps take
+//    turns at staging block it+NS-1; completion is tracked by cp.async.mbarrier.arrive.
+//  * Order across chains: chain-major (R5), as in the other kernels.
+#pragma once
+#include "bt_common.cuh"
+
+namespace elpa2bt {
+
+template <int NBW_>
+struct WyCfg {
+    static constexpr int NBW = NBW_;
+    static constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    static constexpr int NT = NBW / 8 + 1;            // 8-row tiles in the window
+    static constexpr int W = 8 * NT;                  // window rows (= nbw + 8; W % 16 == 8)
+    static constexpr int NW = 8;                      // warps per CTA
+    static constexpr int NGMAX = (NBW <= 64) ? 4 : 2; // most 8-column slabs per warp
+    static constexpr int NS = 4;                      // ring stages
+    static constexpr int VA_OFF = 0;                  // VA[i][w], row stride W
+    static constexpr int VB_OFF = 8 * W;              // VB[w][i], row stride 8
+    static constexpr int TN_OFF = 16 * W;             // TN[n][k] = -T[n][k]
+    static constexpr int STAGE_DOUBLES = 16 * W + 64;
+    static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
+    static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
+    static_assert(W % 16 == 8, "VA row stride must be 8 mod 16 doubles (bank-conflict-free LDS.128)");
+};
+
+struct WyArgs {
+    int64_t N, nev, ldq;
+    const double *hh_v;    // G * nbw
+    const double *hh_tau;  // G
+    double *q;
+    double *tn;            // scratch: 64 doubles (-T, row-major) per block, in consumption order
+    int align16;           // q base and ldq*8 are 16-byte aligned
+};
+
+// ---- block enumeration ----------------------------------------------------------------------------
+// chain k = 0 .. K0-1 (K0 = ceil((N-1)/nbw)); within a chain, blocks b = bhi down to k*nbw/8, where
+// bhi = (N-1)/8.  id(k, b) = base(k) + (bhi - b) is the consumption order.
+__host__ __device__ __forceinline__ int64_t wy_bhi(int64_t N) { return (N - 1) >> 3; }
+__host__ __device__ __forceinline__ int64_t wy_base(int64_t N, int lg, int64_t k)
+{
+    return k * (wy_bhi(N) + 1) - ((int64_t)1 << (lg - 3)) * ((k * (k - 1)) >> 1);
+}
+__host__ __device__ __forceinline__ int64_t wy_nchains(int64_t N, int lg) { return (N - 2 + ((int64_t)1 << lg)) >> lg; }
+__host__ __device__ __forceinline__ int64_t wy_nblocks(int64_t N, int lg) { return wy_base(N, lg, wy_nchains(N, lg)); }
+
+// slot of reflector i of block (k, b) (first row r0 = 8b + 7 - i; sweep s = r0 - 1 - k nbw; R3),
+// -1 if the block position is outside the chain
+template <int LG>
+__device__ __forceinline__ int64_t wy_slot(int64_t N, int64_t FN1, int64_t k, int64_t b, int i)
+{
+    const int64_t r0 = (b << 3) + 7 - i;
+    const int64_t s = r0 - 1 - (k << LG);
+    if (r0 > N - 1 || s < 0) return -1;
+    return FN1 - hh_F(N - 1 - s, LG) + k;
+}
+
+__device__ __forceinline__ void dmma884(double &d0, double &d1, const double a, const double b, const double c0,
+                                        const double c1)
+{
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%5};"
+        : "=d"(d0), "=d"(d1)
+        : "d"(a), "d"(b), "d"(c0), "d"(c1));
+}
+
+__device__ __forceinline__ void cp_async_mbar_arrive_noinc_wy(uint32_t bar)
+{
+    asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// ---- prepass: -T of every block -------------------------------------------------------------------
+// grid (ceil((bhi+1)/8), K0), 256 threads: warp = one block (k, b).  Lane (gq, r) loads column gq
+// of V at window rows 4c + r, c = 0 .. W/4-1 (both the A and the B fragment of V^T V), the Gram
+// matrix comes out of W/4 DMMAs, then lane l & 7 runs the recurrence for column l of T.
+template <int NBW>
+__global__ void __launch_bounds__(256) wy_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
+                                                         const double *__restrict__ hh_tau, double *__restrict__ tn)
+{
+    using C = WyCfg<NBW>;
+    __shared__ double Sm[8][64];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int gq = lane >> 2, r = lane & 3;
+    const int64_t k = blockIdx.y;
+    const int64_t bhi = wy_bhi(N);
+    const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
+    const int64_t j = (int64_t)blockIdx.x * 8 + warp;
+    if (j >= nblk) return;
+    const int64_t b = bhi - j;
+    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t slot = wy_slot<C::LG>(N, FN1, k, b, gq);
+    const double tau = slot >= 0 ? hh_tau[slot] : 0.0;
+    double s0 = 0.0, s1 = 0.0, u0 = 0.0, u1 = 0.0;
+#pragma unroll
+    for (int c = 0; c < C::W / 4; ++c) {
+        const int rl = 4 * c + r - (7 - gq);
+        const double v = (slot >= 0 && rl >= 0 && rl < NBW) ? hh_v[slot * NBW + rl] : 0.0;
+        if (c & 1)
+            dmma884(u0, u1, v, v, u0, u1);
+        else
+            dmma884(s0, s1, v, v, s0, s1);
+    }
+    // S[m = gq][n = 2r + {0,1}]
+    Sm[warp][gq * 8 + 2 * r] = s0 + u0;
+    Sm[warp][gq * 8 + 2 * r + 1] = s1 + u1;
+    __syncwarp();
+    const int l = lane & 7;
+    double t[8];
+#pragma unroll
+    for (int jj = 0; jj < 8; ++jj) {
+        const double tau_j = __shfl_sync(0xffffffffu, tau, 4 * jj);
+        double acc = 0.0;
+#pragma unroll
+        for (int i = 0; i < jj; ++i) acc = fma(Sm[warp][jj * 8 + i], t[i], acc);
+        t[jj] = (jj == l) ? tau_j : (jj > l ? -tau_j * acc : 0.0);
+    }
+    double *out = tn + (wy_base(N, C::LG, k) + j) * 64;
+    if (lane < 8) {
+#pragma unroll
+        for (int jj = 0; jj < 8; ++jj) out[jj * 8 + l] = -t[jj];
+    }
+}
+
+// ---- staging one block (whole warp) -----------------------------------------------------------------
+template <class C>
+__device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_t bar_full, int64_t k, int64_t b,
+                                         int64_t id, int64_t FN1, int lane)
+{
+    constexpr int NBW = C::NBW, W = C::W;
+    const int i8 = lane & 7;
+    const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
+    // VA[i][7 - i + r]: lanes run along r (256 contiguous bytes of hh_v per instruction)
+#pragma unroll
+    for (int t = 0; t < 8 * NBW / 32; ++t) {
+        const int i = (t * 32) / NBW;
+        const int rr = (t * 32) % NBW + lane;
+        const int64_t sl = __shfl_sync(0xffffffffu, slot, i);
+        if (sl >= 0) cp_async8(smem_u32(stage + C::VA_OFF + i * W + 7 - i + rr), a.hh_v + sl * NBW + rr, 8u);
+    }
+    // VB[7 - i + r][i]: lanes run along i (bank-conflict-light writes), 4 rows per instruction
+    if (slot >= 0) {
+#pragma unroll
+        for (int t = 0; t < NBW / 4; ++t) {
+            const int rr = t * 4 + (lane >> 3);
+            cp_async8(smem_u32(stage + C::VB_OFF + (7 - i8 + rr) * 8 + i8), a.hh_v + slot * NBW + rr, 8u);
+        }
+    }
+    cp_async16(smem_u32(stage + C::TN_OFF + 2 * lane), a.tn + id * 64 + 2 * lane, 16u);
+    cp_async_mbar_arrive_noinc_wy(bar_full);
+}
+
+// ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column ------------------------------------------
+__device__ __forceinline__ void wy_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &x0,
+                                         double &x1)
+{
+    x0 = 0.0;
+    x1 = 0.0;
+    if (!colok || row >= a.N) return;
+    if (a.align16 && row + 1 < a.N) {
+        const double2 v = *reinterpret_cast<const double2 *>(colp + row);
+        x0 = v.x;
+        x1 = v.y;
+    } else {
+        x0 = colp[row];
+        if (row + 1 < a.N) x1 = colp[row + 1];
+    }
+}
+__device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double x0, double x1)
+{
+    if (!colok || row >= a.N) return;
+    if (a.align16 && row + 1 < a.N) {
+        *reinterpret_cast<double2 *>(colp + row) = make_double2(x0, x1);
+    } else {
+        colp[row] = x0;
+        if (row + 1 < a.N) colp[row + 1] = x1;
+    }
+}
+
+// ---- a warp with NG slabs of 8 columns ---------------------------------------------------------------
+template <class C, int NG>
+__device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int warp, const int lane,
+                                           const int nact, const int64_t col0)
+{
+    constexpr int NT = C::NT, W = C::W, NS = C::NS, NBW = C::NBW;
+    constexpr int NACC = (NG >= 3) ? 1 : 2;          // dot-product accumulator sets per slab
+    double *ring = reinterpret_cast<double *>(smem);
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + NS * 8;
+    const int gq = lane >> 2, r = lane & 3;
+    const int64_t N = a.N;
+    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t bhi = wy_bhi(N);
+    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t nblocks = wy_nblocks(N, C::LG);
+
+    double *colp[NG];
+    bool colok[NG];
+#pragma unroll
+    for (int g = 0; g < NG; ++g) {
+        const int64_t col = col0 + 8 * g + gq;
+        colok[g] = col < a.nev;
+        colp[g] = a.q + (colok[g] ? col : 0) * a.ldq;
+    }
+
+    // staging cursor: block it + NS - 1
+    int64_t pk = 0, pb = bhi;
+    auto advance = [&]() {
+        if (pb > (pk << (C::LG - 3))) {
+            --pb;
+        } else {
+            ++pk;
+            pb = bhi;
+        }
+    };
+    if (warp == 0) {
+        for (int i = 0; i < NS - 1; ++i) {
+            if (i < nblocks) wy_stage<C>(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pk, pb, i, FN1, lane);
+            advance();
+        }
+    } else {
+        for (int i = 0; i < NS - 1; ++i) advance();
+    }
+
+    double X[NG][NT + 1][2];
+    int64_t it = 0;
+    uint32_t duty = 0;
+    for (int64_t k = 0; k < K0; ++k) {
+        const int64_t blo = k << (C::LG - 3);
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+#pragma unroll
+            for (int t = 1; t <= NT; ++t) X[g][t][0] = X[g][t][1] = 0.0;
+            wy_load2(a, colp[g], colok[g], (bhi << 3) + 2 * r, X[g][0][0], X[g][0][1]);
+        }
+        for (int64_t b = bhi; b >= blo; --b, ++it) {
+            // --- staging duty: block it+NS-1 goes into the stage that block it-1 used
+            if (duty == (uint32_t)warp) {
+                const int64_t jt = it + NS - 1;
+                if (jt < nblocks) {
+                    const uint32_t st = (uint32_t)(jt % NS);
+                    if (it >= 1) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - 1) / NS) & 1));
+                    wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, jt, FN1, lane);
+                }
+            }
+            advance();
+            duty = (duty + 1 == (uint32_t)nact) ? 0 : duty + 1;
+
+            const uint32_t st = (uint32_t)(it % NS), ph = (uint32_t)((it / NS) & 1);
+            mbar_wait(bar_full + 8 * st, ph);
+            const double *stage = ring + st * C::STAGE_DOUBLES;
+            const double *va = stage + C::VA_OFF + gq * W + 2 * r;
+            const double *vb = stage + C::VB_OFF + gq * 8 + 2 * r;
+            const double *tn = stage + C::TN_OFF + gq * 8 + 2 * r;
+
+            // --- D^T = x^T V: k-chunk (t, e) = rows 8t + 2r' + e; tile 0 (loaded last) goes last
+            double D[NG][NACC][2];
+#pragma unroll
+            for (int g = 0; g < NG; ++g)
+#pragma unroll
+                for (int s = 0; s < NACC; ++s) D[g][s][0] = D[g][s][1] = 0.0;
+#pragma unroll
+            for (int tt = 0; tt < NT; ++tt) {
+                const int t = (tt + 1) % NT;
+                const double2 v2 = *reinterpret_cast<const double2 *>(va + 8 * t);
+#pragma unroll
+                for (int g = 0; g < NG; ++g)
+                    dmma884(D[g][0][0], D[g][0][1], X[g][t][0], v2.x, D[g][0][0], D[g][0][1]);
+#pragma unroll
+                for (int g = 0; g < NG; ++g)
+                    dmma884(D[g][NACC - 1][0], D[g][NACC - 1][1], X[g][t][1], v2.y, D[g][NACC - 1][0], D[g][NACC - 1][1]);
+            }
+            // --- E^T = D^T (-T)^T
+            double E[NG][2];
+            {
+                const double2 t2 = *reinterpret_cast<const double2 *>(tn);
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+                    double d0 = D[g][0][0], d1 = D[g][0][1];
+                    if (NACC == 2) {
+                        d0 += D[g][1][0];
+                        d1 += D[g][1][1];
+                    }
+                    double e0, e1;
+                    dmma884(e0, e1, d0, t2.x, 0.0, 0.0);
+                    dmma884(E[g][0], E[g][1], d1, t2.y, e0, e1);
+                }
+            }
+            // --- x^T += E^T V^T, tile t -> registers of tile t+1 (the window moves up by 8 rows)
+#pragma unroll
+            for (int t = NT - 1; t >= 0; --t) {
+                const double2 v2 = *reinterpret_cast<const double2 *>(vb + 64 * t);
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+                    double m0, m1;
+                    dmma884(m0, m1, E[g][0], v2.x, X[g][t][0], X[g][t][1]);
+                    dmma884(X[g][t + 1][0], X[g][t + 1][1], E[g][1], v2.y, m0, m1);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8 * st);
+            // --- tile NT-1 retires (rows 8b + nbw ..), tile 0 of the next block comes in
+#pragma unroll
+            for (int g = 0; g < NG; ++g) {
+                wy_store2(a, colp[g], colok[g], (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
+                if (b > blo)
+                    wy_load2(a, colp[g], colok[g], ((b - 1) << 3) + 2 * r, X[g][0][0], X[g][0][1]);
+            }
+        }
+        // --- chain end: tiles 1 .. NT-1 hold rows 8 blo + 8 (t-1) + 2r + {0,1}
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+#pragma unroll
+            for (int t = 1; t < NT; ++t)
+                wy_store2(a, colp[g], colok[g], (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
+    }
+}
+
+// ---- the kernel ----------------------------------------------------------------------------------------
+// grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid) (at most NW*NGMAX of them); warp w takes
+// n/NW of those, +1 for the first n%NW warps (warps w and w+4 share a sub-partition, so the extras
+// land on different sub-partitions first).
+template <int NBW>
+__global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
+{
+    using C = WyCfg<NBW>;
+    constexpr int NS = C::NS, NW = C::NW, NGMAX = C::NGMAX;
+    extern __shared__ __align__(128) unsigned char smem[];
+    double *ring = reinterpret_cast<double *>(smem);
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + NS * 8;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t nslab = (a.nev + 7) >> 3;
+    const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
+    const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
+    const int nact = nmine < NW ? nmine : NW;
+    const int base = nmine / NW, extra = nmine % NW;
+    const int ng = base + (warp < extra ? 1 : 0);
+    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
+
+    // the ring starts as zeros: the skew padding of VA / VB is never written by the copies, and
+    // positions of reflectors outside a chain keep finite values (their row and column of T are 0)
+    for (int i = threadIdx.x; i < C::OFF_BAR / 8; i += blockDim.x) ring[i] = 0.0;
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(bar_full + 8 * i, 32);           // one cp.async arrival per lane of the staging warp
+            mbar_init(bar_empty + 8 * i, (uint32_t)nact);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (ng == 0) return;
+
+    const int64_t col0 = wslab0 << 3;
+    if (NGMAX >= 4 && ng == 4)
+        wy_consume<C, (NGMAX >= 4 ? 4 : 1)>(a, smem, warp, lane, nact, col0);
+    else if (NGMAX >= 3 && ng == 3)
+        wy_consume<C, (NGMAX >= 3 ? 3 : 1)>(a, smem, warp, lane, nact, col0);
+    else if (ng == 2)
+        wy_consume<C, 2>(a, smem, warp, lane, nact, col0);
+    else
+        wy_consume<C, 1>(a, smem, warp, lane, nact, col0);
+}
+
+// ---- host side -----------------------------------------------------------------------------------------
+// bytes of -T scratch the two kernels share
+template <int NBW>
+size_t wy_scratch_bytes(int64_t N)
+{
+    return (size_t)wy_nblocks(N, WyCfg<NBW>::LG) * 64 * sizeof(double);
+}
+
+template <int NBW>
+cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+                      int align16, int nsm, double *tn_scratch, cudaStream_t st, int *launches)
+{
+    using C = WyCfg<NBW>;
+    auto kern = bt_wy_kernel<NBW>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t K0 = wy_nchains(N, C::LG);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
+    wy_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const int64_t nslab = (nev + 7) >> 3;
+    const int64_t per_cta = (int64_t)C::NW * C::NGMAX;
+    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
+    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
+    if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that
+    WyArgs a;
+    a.N = N;
+    a.nev = nev;
+    a.ldq = ldq;
+    a.hh_v = hh_v;
+    a.hh_tau = hh_tau;
+    a.q = q;
+    a.tn = tn_scratch;
+    a.align16 = align16;
+    kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
+    if (launches) *launches = 2;
+    return cudaGetLastError();
+}
+
+}  // namespace elpa2bt

@@ -1,6 +1,7 @@
 // elpa2_bt.cu -- C-ABI entry points of include/elpa2_bt.h: argument validation, launch planning,
-// host-buffer wrapper and the FP64 peak probe.  All arithmetic of the path is in the kernels
-// (bt_window.cuh, bt_simple.cuh).  No torch types, no CPU fallback.
+// host-buffer wrapper.  All arithmetic of the path is in the kernels (bt_wy.cuh: real, DMMA
+// compact-WY; bt_shift.cuh: complex, register window; bt_simple.cuh: plain A/B baseline).
+// No torch types, no CPU fallback.
 #include "../../include/elpa2_bt.h"
 
 #include <cuda_runtime.h>
@@ -9,7 +10,7 @@
 
 #include "bt_shift.cuh"
 #include "bt_simple.cuh"
-#include "bt_window.cuh"
+#include "bt_wy.cuh"
 
 using namespace elpa2bt;
 
@@ -21,7 +22,8 @@ namespace {
 
 int g_variant = 0;
 thread_local int g_last_launches = 0;
-std::mutex g_mu;
+std::mutex g_mu;        // host-buffer entry point (its cached device scratch)
+std::mutex g_pool_mu;   // creation of the scratch pool
 
 int lg_of(int nbw) { return nbw == 32 ? 5 : nbw == 64 ? 6 : nbw == 128 ? 7 : -1; }
 
@@ -39,44 +41,8 @@ int sm_count()
     return n;
 }
 
-// threads per CTA: 7 consumer warps + 1 producer warp = 256 threads, so that each thread may use
-// up to 255 registers (the window, CPL columns x 16 rows per lane, takes 128 of them).  With 9
-// warps (224 registers) ptxas serialises the columns of a step and the kernel is 25 % slower.
-template <bool CPLX, int NBW, int CPL>
-cudaError_t launch_window(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
-                          int64_t ldq, int align16, cudaStream_t st)
-{
-    using C = WinCfg<CPLX, NBW, CPL>;
-    constexpr int MAXT = 256;
-    auto kern = bt_window_kernel<CPLX, NBW, CPL, MAXT>;
-    static bool attr_done = false;
-    constexpr int NWMAX = MAXT / 32 - 1;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)C::smem_bytes(NWMAX));
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
-    const int64_t units = (nev + C::CW - 1) / C::CW;
-    const int64_t nsm = sm_count();
-    const int64_t waves = (units + nsm * NWMAX - 1) / (nsm * NWMAX);
-    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
-    if (grid > units) grid = units;                   // ... unless there are fewer warp-units
-    const int64_t nw = (units + grid - 1) / grid;     // the kernel splits the units evenly over CTAs
-    WinArgs a;
-    a.N = N;
-    a.nev = nev;
-    a.ldq = ldq;
-    a.hh_v = hh_v;
-    a.hh_tau = hh_tau;
-    a.q = q;
-    a.nw = (int)nw;
-    a.align16 = align16;
-    kern<<<(unsigned)grid, (unsigned)((nw + 1) * 32), C::smem_bytes((int)nw), st>>>(a);
-    return cudaGetLastError();
-}
-
-// the shift kernel: same CTA shape (7 consumer warps + 1 producer warp, up to 255 registers)
+// the shift kernel: 7 consumer warps + 1 producer warp = 256 threads, so that each thread may use
+// up to 255 registers (the window, CPL columns x RL rows per lane, takes 128 of them)
 template <bool CPLX, int NBW, int CPL>
 cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q,
                          int64_t ldq, int align16, cudaStream_t st)
@@ -111,6 +77,47 @@ cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const doubl
     return cudaGetLastError();
 }
 
+// stream-ordered scratch for the -T factors of the WY kernel: a private memory pool that keeps
+// what it has allocated (release threshold = max), so that in steady state a call allocates
+// nothing new and never synchronises the host
+cudaMemPool_t scratch_pool(cudaError_t *err)
+{
+    static cudaMemPool_t pool = nullptr;
+    static int pool_dev = -1;
+    int dev = 0;
+    *err = cudaGetDevice(&dev);
+    if (*err != cudaSuccess) return nullptr;
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (pool && pool_dev == dev) return pool;
+    cudaMemPoolProps props = {};
+    props.allocType = cudaMemAllocationTypePinned;
+    props.handleTypes = cudaMemHandleTypeNone;
+    props.location.type = cudaMemLocationTypeDevice;
+    props.location.id = dev;
+    cudaMemPool_t p = nullptr;
+    *err = cudaMemPoolCreate(&p, &props);
+    if (*err != cudaSuccess) return nullptr;
+    uint64_t keep = UINT64_MAX;
+    cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+    pool = p;
+    pool_dev = dev;
+    return pool;
+}
+
+template <int NBW>
+cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+                   int align16, cudaStream_t st)
+{
+    cudaError_t e;
+    cudaMemPool_t pool = scratch_pool(&e);
+    if (!pool) return e;
+    void *tn = nullptr;
+    if ((e = cudaMallocFromPoolAsync(&tn, wy_scratch_bytes<NBW>(N), pool, st)) != cudaSuccess) return e;
+    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), (double *)tn, st, nullptr);
+    const cudaError_t e2 = cudaFreeAsync(tn, st);
+    return e != cudaSuccess ? e : e2;
+}
+
 template <bool CPLX>
 int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
         void *stream)
@@ -131,27 +138,29 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
     if (((uintptr_t)q & (8 * EW - 1)) != 0) return -6;
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e;
+    int nlaunch = 1;
     if (g_variant == 1) {
         const unsigned grid = (unsigned)((nev + 127) / 128);
         bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
         e = cudaGetLastError();
-    } else if (g_variant == 0) {
+    } else if (g_variant == 0 && !CPLX) {
+        const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
+        switch (nbw) {
+        case 32: e = run_wy<32>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 64: e = run_wy<64>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        default: e = run_wy<128>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        }
+        nlaunch = 2;
+    } else {
         const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
         switch (nbw) {
         case 32: e = launch_shift<CPLX, 32, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
         case 64: e = launch_shift<CPLX, 64, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
         default: e = launch_shift<CPLX, 128, 2>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
         }
-    } else {
-        const int align16 = CPLX ? 1 : ((((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0);
-        switch (nbw) {
-        case 32: e = launch_window<CPLX, 32, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        case 64: e = launch_window<CPLX, 64, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        default: e = launch_window<CPLX, 128, CPLX ? 2 : 4>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        }
     }
     if (e != cudaSuccess) return (int)e;
-    g_last_launches = 1;
+    g_last_launches = nlaunch;
     return 0;
 }
 

@@ -123,7 +123,7 @@ def test_host_entry_point(cplx):
     y = np.array(x, order="F", copy=True)
     binding.trans_ev_tridi_to_band_host(N, nbw, hh_v, hh_tau, y)
     assert np.abs(y - want).max() <= TOL * np.abs(x).max()
-    assert binding.last_launch_count() == 1
+    assert binding.last_launch_count() == (1 if cplx else 2)     # real: prepass + main kernel
 
 
 def test_launch_on_side_stream():
