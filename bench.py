@@ -5,7 +5,8 @@ on synthetic inputs of BASELINE.json's shapes.
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
 
 One "step" = one call of ``elpa2_trans_ev_tridi_to_band_{d,z}`` over the whole N x nev block (all
-SURVEY.md 8(a) rows a1-a5 happen inside that one kernel launch).  Default workload: config 4
+SURVEY.md 8(a) rows a1-a6 happen inside that call: real = T-factor prepass + compact-WY DMMA
+kernel, complex = one register-window kernel).  Default workload: config 4
 (real FP64, N = 32768, nbw = 64, nev = 32768), the configuration BASELINE.json's target is quoted
 on.  Reflectors for the timed run are the seeded synthetic unitary stream of
 ``synth_inputs.synthetic_reflectors`` (same layout, lengths, tau != 0 pattern and value range as
@@ -249,8 +250,13 @@ def main() -> None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    # ---- FP64 ALU peak of this device, measured live (outside the timed region) ----
+    # ---- FP64 peaks of this device, measured live (outside the timed region): the real path is a
+    #      DMMA (FP64 tensor core) contraction, the complex path plain DFMA arithmetic; both share
+    #      one pipe, so each is judged against its own instruction's probe
     dfma_tf = binding.probe_fp64(0, 8192, 20)
+    dmma_tf = binding.probe_fp64(1, 8192, 20)
+    tensor_path = not cplx
+    peak_tf = dmma_tf if tensor_path else dfma_tf
 
     ncheck = min(nev, 64)
     nrm0 = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
@@ -335,12 +341,16 @@ def main() -> None:
                               % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
                              else "inputs smaller than L2; config is latency-bound (DESIGN.md)",
                        "parallelism": "column shards, no collective" if world > 1 else "single GPU"},
-            "roofline": {"bound": "alu", "achieved": achieved, "peak": dfma_tf, "unit": "TFLOP/s",
-                         "frac": achieved / dfma_tf,
-                         "peak_source": "DFMA probe measured in this run (elpa2_bt_probe_fp64 kind 0); "
-                                        "MEASURED_PEAKS.json has no FP64 figure",
+            "roofline": {"bound": "tensor" if tensor_path else "alu", "achieved": achieved, "peak": peak_tf,
+                         "unit": "TFLOP/s", "frac": achieved / peak_tf,
+                         "peak_source": ("FP64 %s probe measured in this run (elpa2_bt_probe_fp64 kind %d); "
+                                         "MEASURED_PEAKS.json has no FP64 figure"
+                                         % (("DMMA m8n8k4", 1) if tensor_path else ("DFMA", 0))),
+                         "peak_dfma_probe": dfma_tf, "peak_dmma_probe": dmma_tf,
                          "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                         "kernel": "bt_shift_kernel", "kernel_ms": kern_ms,
+                         "kernel": ("bt_wy_kernel (the interval also holds its wy_prepass_kernel)"
+                                    if tensor_path else "bt_shift_kernel"),
+                         "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
                          "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},

@@ -27,7 +27,7 @@
 //    breaks the 16-byte alignment bulk copies need); -T comes from a scratch array filled by
 //    wy_prepass_kernel (one warp per block: Gram matrix V^T V by DMMA, then the recurrence).
 //  * 8 warps per CTA (2 per SM sub-partition, 255 registers), no producer warp: the warps take
-//    turns at staging block it+NS-1; completion is tracked by cp.async.mbarrier.arrive.
+//    turns at staging block it+NS-LAG; completion is tracked by cp.async.mbarrier.arrive.
 //  * Order across chains: chain-major (R5), as in the other kernels.
 #pragma once
 #include "bt_common.cuh"
@@ -42,7 +42,8 @@ struct WyCfg {
     static constexpr int W = 8 * NT;                  // window rows (= nbw + 8; W % 16 == 8)
     static constexpr int NW = 8;                      // warps per CTA
     static constexpr int NGMAX = (NBW <= 64) ? 4 : 2; // most 8-column slabs per warp
-    static constexpr int NS = 4;                      // ring stages
+    static constexpr int NS = 8;                      // ring stages
+    static constexpr int LAG = 4;                     // staging waits for the block LAG iterations back
     static constexpr int VA_OFF = 0;                  // VA[i][w], row stride W
     static constexpr int VB_OFF = 8 * W;              // VB[w][i], row stride 8
     static constexpr int TN_OFF = 16 * W;             // TN[n][k] = -T[n][k]
@@ -208,7 +209,7 @@ template <class C, int NG>
 __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int warp, const int lane,
                                            const int nact, const int64_t col0)
 {
-    constexpr int NT = C::NT, W = C::W, NS = C::NS, NBW = C::NBW;
+    constexpr int NT = C::NT, W = C::W, NS = C::NS, NBW = C::NBW, LAG = C::LAG;
     constexpr int NACC = (NG >= 3) ? 1 : 2;          // dot-product accumulator sets per slab
     double *ring = reinterpret_cast<double *>(smem);
     const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
@@ -220,16 +221,12 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const int64_t FN1 = hh_F(N - 1, C::LG);
     const int64_t nblocks = wy_nblocks(N, C::LG);
 
-    double *colp[NG];
-    bool colok[NG];
-#pragma unroll
-    for (int g = 0; g < NG; ++g) {
-        const int64_t col = col0 + 8 * g + gq;
-        colok[g] = col < a.nev;
-        colp[g] = a.q + (colok[g] ? col : 0) * a.ldq;
-    }
+    // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1
+    double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq;
+    const int64_t ldq8 = a.ldq << 3;
+    const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
 
-    // staging cursor: block it + NS - 1
+    // staging cursor: block it + NS - LAG
     int64_t pk = 0, pb = bhi;
     auto advance = [&]() {
         if (pb > (pk << (C::LG - 3))) {
@@ -239,13 +236,14 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             pb = bhi;
         }
     };
+    // prologue: blocks 0 .. NS-LAG-1 go into fresh stages
     if (warp == 0) {
-        for (int i = 0; i < NS - 1; ++i) {
+        for (int i = 0; i < NS - LAG; ++i) {
             if (i < nblocks) wy_stage<C>(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pk, pb, i, FN1, lane);
             advance();
         }
     } else {
-        for (int i = 0; i < NS - 1; ++i) advance();
+        for (int i = 0; i < NS - LAG; ++i) advance();
     }
 
     double X[NG][NT + 1][2];
@@ -257,15 +255,16 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
         for (int g = 0; g < NG; ++g) {
 #pragma unroll
             for (int t = 1; t <= NT; ++t) X[g][t][0] = X[g][t][1] = 0.0;
-            wy_load2(a, colp[g], colok[g], (bhi << 3) + 2 * r, X[g][0][0], X[g][0][1]);
+            wy_load2(a, cb + g * ldq8, 8 * g < ncolrem, (bhi << 3) + 2 * r, X[g][0][0], X[g][0][1]);
         }
         for (int64_t b = bhi; b >= blo; --b, ++it) {
-            // --- staging duty: block it+NS-1 goes into the stage that block it-1 used
+            // --- staging duty: block it+NS-LAG goes into the stage that block it-LAG used; the warp
+            //     on duty only waits if some warp is still LAG blocks behind it
             if (duty == (uint32_t)warp) {
-                const int64_t jt = it + NS - 1;
+                const int64_t jt = it + NS - LAG;
                 if (jt < nblocks) {
                     const uint32_t st = (uint32_t)(jt % NS);
-                    if (it >= 1) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - 1) / NS) & 1));
+                    if (it >= LAG) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - LAG) / NS) & 1));
                     wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, jt, FN1, lane);
                 }
             }
@@ -328,9 +327,9 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             // --- tile NT-1 retires (rows 8b + nbw ..), tile 0 of the next block comes in
 #pragma unroll
             for (int g = 0; g < NG; ++g) {
-                wy_store2(a, colp[g], colok[g], (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
+                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
                 if (b > blo)
-                    wy_load2(a, colp[g], colok[g], ((b - 1) << 3) + 2 * r, X[g][0][0], X[g][0][1]);
+                    wy_load2(a, cb + g * ldq8, 8 * g < ncolrem, ((b - 1) << 3) + 2 * r, X[g][0][0], X[g][0][1]);
             }
         }
         // --- chain end: tiles 1 .. NT-1 hold rows 8 blo + 8 (t-1) + 2r + {0,1}
@@ -338,7 +337,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
         for (int g = 0; g < NG; ++g)
 #pragma unroll
             for (int t = 1; t < NT; ++t)
-                wy_store2(a, colp[g], colok[g], (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
+                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
     }
 }
 
