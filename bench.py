@@ -5,8 +5,8 @@ on synthetic inputs of BASELINE.json's shapes.
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 1..5] [--impl reference]
 
 One "step" = one call of ``elpa2_trans_ev_tridi_to_band_{d,z}`` over the whole N x nev block (all
-SURVEY.md 8(a) rows a1-a6 happen inside that call: real = T-factor prepass + compact-WY DMMA
-kernel, complex = one register-window kernel).  Default workload: config 4
+SURVEY.md 8(a) rows a1-a6 happen inside that call: T-factor prepass + compact-WY DMMA
+kernel).  Default workload: config 4
 (real FP64, N = 32768, nbw = 64, nev = 32768), the configuration BASELINE.json's target is quoted
 on.  Reflectors for the timed run are the seeded synthetic unitary stream of
 ``synth_inputs.synthetic_reflectors`` (same layout, lengths, tau != 0 pattern and value range as
@@ -251,11 +251,11 @@ def main() -> None:
         torch.cuda.synchronize()
 
     # ---- FP64 peaks of this device, measured live (outside the timed region): the real path is a
-    #      DMMA (FP64 tensor core) contraction, the complex path plain DFMA arithmetic; both share
-    #      one pipe, so each is judged against its own instruction's probe
+    #      path is a DMMA (FP64 tensor core) contraction, judged against the DMMA probe; the DFMA
+    #      probe (the same pipe) is reported beside it
     dfma_tf = binding.probe_fp64(0, 8192, 20)
     dmma_tf = binding.probe_fp64(1, 8192, 20)
-    tensor_path = not cplx
+    tensor_path = True
     peak_tf = dmma_tf if tensor_path else dfma_tf
 
     ncheck = min(nev, 64)
@@ -348,8 +348,8 @@ def main() -> None:
                                          % (("DMMA m8n8k4", 1) if tensor_path else ("DFMA", 0))),
                          "peak_dfma_probe": dfma_tf, "peak_dmma_probe": dmma_tf,
                          "peak_nominal": NOMINAL_FP64_TFLOPS, "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                         "kernel": ("bt_wy_kernel (the interval also holds its wy_prepass_kernel)"
-                                    if tensor_path else "bt_shift_kernel"),
+                         "kernel": ("bt_wyz_kernel" if cplx else "bt_wy_kernel")
+                                   + " (the interval also holds its T-factor prepass kernel)",
                          "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
                          "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,

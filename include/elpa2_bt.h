@@ -27,8 +27,10 @@
  * Ownership and execution: the caller owns every buffer.  hh_v, hh_tau and q are DEVICE pointers
  * valid on the current CUDA device; hh_* are read-only.  The call enqueues work on `stream`
  * (a cudaStream_t passed as void*; NULL = the legacy default stream), returns without
- * synchronising the host, and allocates nothing (keep data on the device, no
- * implicit synchronisation).  There is no CPU fallback: without a CUDA device every compute call
+ * synchronising the host (keep data on the device, no implicit synchronisation).
+ * The default variant takes its scratch (64 / 128 doubles per block of 8 reflectors, about
+ * N^2/(16 nbw) blocks) from a stream-ordered CUDA memory pool private to the library, which keeps
+ * what it has allocated: in steady state a call allocates nothing new.  There is no CPU fallback: without a CUDA device every compute call
  * fails with the cudaError_t of the launch.
  *
  * Return value: 0 on success; -i if the i-th argument (1-based: N=1, nbw=2, nev=3, hh_v=4,
@@ -74,9 +76,12 @@ int64_t elpa2_hh_offset(int64_t N, int nbw, int64_t s);
 int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
 
 /* Kernels launched by the last successful compute call of this thread's library state (for
- * bench.py's "gpu_launches"), and a selector for A/B runs: variant 0 = default (fastest),
- * 1 = simple shared-memory-window kernel (correctness baseline).  Returns the previous variant
- * or -1 if `variant` is unknown. */
+ * bench.py's "gpu_launches"), and a selector for A/B runs: variant 0 = default (compact-WY
+ * aggregation of 8 reflectors on the FP64 tensor cores, R6: a T-factor prepass kernel + the main
+ * kernel = 2 launches; its scratch comes from a stream-ordered pool that keeps its memory),
+ * 1 = plain kernel (one thread per column, literal reverse generation order), 2 = one reflector at
+ * a time in a register-resident window (DFMA, 1 launch).  Returns the previous variant or -1 if
+ * `variant` is unknown. */
 int elpa2_bt_last_launch_count(void);
 int elpa2_bt_set_variant(int variant);
 

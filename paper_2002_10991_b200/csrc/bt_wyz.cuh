@@ -1,0 +1,400 @@
+// bt_wyz.cuh -- compact-WY back-transformation on the FP64 tensor cores, COMPLEX FP64 (sm_100a).
+// Same algorithm and fragment chaining as bt_wy.cuh; every complex product is four real DMMAs.
+//
+//      H_7 .. H_0 = I - V T V^H,  T lower triangular, T[j][j] = tau_j,
+//      T[j][:j] = -tau_j (v_j^H V[:, :j]) T[:j, :j]                    (R2: tau as stored, v^H in the dot)
+//      D^T = x^T conj(V):  Dr = xr Vr + xi Vi,  Di = xi Vr - xr Vi      (four accumulators, 4 chains)
+//      E^T = D^T (-T)^T:   Er = Dr TNr - Di TNi, Ei = Dr TNi + Di TNr
+//      x^T += E^T V^T:     xr += Er Vr - Ei Vi,  xi += Er Vi + Ei Vr
+// Registers hold x planar (real and imaginary fragments apart); global memory and shared memory
+// stay interleaved (re, im): one LDS.128 / LDG.128 = one complex element.  Interleaved 16-byte
+// elements keep the skewed rows of VA 16-byte aligned, so VA is staged with one bulk copy (TMA
+// engine) per reflector; VB (the transposed image) and -T by 16-byte cp.async.
+#pragma once
+#include "bt_wy.cuh"
+
+namespace elpa2bt {
+
+template <int NBW_>
+struct WyzCfg {
+    static constexpr int NBW = NBW_;
+    static constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    static constexpr int NT = NBW / 8 + 1;            // 8-row tiles in the window
+    static constexpr int W = 8 * NT;                  // window rows
+    static constexpr int NW = 8;                      // warps per CTA
+    static constexpr int NGMAX = (NBW <= 64) ? 2 : 1; // most 8-column slabs per warp
+    static constexpr int NS = (NBW <= 64) ? 8 : 4;    // ring stages
+    static constexpr int LAG = NS / 2;                // staging waits for the block LAG iterations back
+    // element = 2 doubles.  Row strides padded by one element: rows gq and gq+1 of a quarter-warp
+    // then differ by 4 banks (W*4 and 8*4 words are multiples of 32)
+    static constexpr int SA = W + 1;                  // VA[i][w] row stride (elements)
+    static constexpr int SB = 9;                      // VB[w][i] row stride (elements)
+    static constexpr int VA_OFF = 0;                  // offsets in doubles
+    static constexpr int VB_OFF = 2 * 8 * SA;
+    static constexpr int TN_OFF = VB_OFF + 2 * W * SB;
+    static constexpr int STAGE_DOUBLES = ((TN_OFF + 128 + 15) / 16) * 16;
+    static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
+    static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
+    static_assert((VB_OFF * 8) % 16 == 0 && (TN_OFF * 8) % 16 == 0, "16-byte aligned sections");
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
+};
+
+// ---- prepass: -T of every block (128 doubles: [n][k] interleaved) --------------------------------------
+template <int NBW>
+__global__ void __launch_bounds__(256) wyz_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
+                                                          const double *__restrict__ hh_tau, double *__restrict__ tn)
+{
+    using C = WyzCfg<NBW>;
+    __shared__ double Sm[8][128];
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int gq = lane >> 2, r = lane & 3;
+    const int64_t k = blockIdx.y;
+    const int64_t bhi = wy_bhi(N);
+    const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
+    const int64_t j = (int64_t)blockIdx.x * 8 + warp;
+    if (j >= nblk) return;
+    const int64_t b = bhi - j;
+    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t slot = wy_slot<C::LG>(N, FN1, k, b, gq);
+    double taur = 0.0, taui = 0.0;
+    if (slot >= 0) {
+        taur = hh_tau[2 * slot];
+        taui = hh_tau[2 * slot + 1];
+    }
+    // S = V^H V:  Sr = Vr^T Vr + Vi^T Vi,  Si = Vr^T Vi - Vi^T Vr
+    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0, p0 = 0.0, p1 = 0.0, q0 = 0.0, q1 = 0.0;
+#pragma unroll
+    for (int c = 0; c < C::W / 4; ++c) {
+        const int rl = 4 * c + r - (7 - gq);
+        double vr = 0.0, vi = 0.0;
+        if (slot >= 0 && rl >= 0 && rl < NBW) {
+            const double2 v2 = *reinterpret_cast<const double2 *>(hh_v + (slot * NBW + rl) * 2);
+            vr = v2.x;
+            vi = v2.y;
+        }
+        dmma884(a0, a1, vr, vr, a0, a1);
+        dmma884(b0, b1, vi, vi, b0, b1);
+        dmma884(p0, p1, vr, vi, p0, p1);
+        dmma884(q0, q1, vi, vr, q0, q1);
+    }
+    // S[m = gq][n = 2r + {0,1}]
+    Sm[warp][(gq * 8 + 2 * r) * 2] = a0 + b0;
+    Sm[warp][(gq * 8 + 2 * r) * 2 + 1] = p0 - q0;
+    Sm[warp][(gq * 8 + 2 * r + 1) * 2] = a1 + b1;
+    Sm[warp][(gq * 8 + 2 * r + 1) * 2 + 1] = p1 - q1;
+    __syncwarp();
+    const int l = lane & 7;
+    double tr[8], ti[8];
+#pragma unroll
+    for (int jj = 0; jj < 8; ++jj) {
+        const double tjr = __shfl_sync(0xffffffffu, taur, 4 * jj);
+        const double tji = __shfl_sync(0xffffffffu, taui, 4 * jj);
+        double ar = 0.0, ai = 0.0;
+#pragma unroll
+        for (int i = 0; i < jj; ++i) {
+            const double sr = Sm[warp][(jj * 8 + i) * 2], si = Sm[warp][(jj * 8 + i) * 2 + 1];
+            ar = fma(sr, tr[i], ar);
+            ar = fma(-si, ti[i], ar);
+            ai = fma(sr, ti[i], ai);
+            ai = fma(si, tr[i], ai);
+        }
+        // -tau_j * acc
+        const double mr = -(tjr * ar - tji * ai), mi = -(tjr * ai + tji * ar);
+        tr[jj] = (jj == l) ? tjr : (jj > l ? mr : 0.0);
+        ti[jj] = (jj == l) ? tji : (jj > l ? mi : 0.0);
+    }
+    double *out = tn + (wy_base(N, C::LG, k) + j) * 128;
+    if (lane < 8) {
+#pragma unroll
+        for (int jj = 0; jj < 8; ++jj)
+            *reinterpret_cast<double2 *>(out + (jj * 8 + l) * 2) = make_double2(-tr[jj], -ti[jj]);
+    }
+}
+
+// ---- staging one block (whole warp) ---------------------------------------------------------------------
+// full barrier: 32 cp.async arrivals (one per lane) + 1 arrival with the bulk-copy byte count
+template <class C>
+__device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32_t bar_full, int64_t k, int64_t b,
+                                          int64_t id, int64_t FN1, int lane)
+{
+    constexpr int NBW = C::NBW;
+    const int i8 = lane & 7;
+    const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
+    // VA[i][7 - i + r]: one bulk copy per reflector (lanes 0..7), nbw * 16 bytes each
+    const unsigned valid = __ballot_sync(0xffffffffu, slot >= 0) & 0xffu;
+    if (lane == 0) mbar_arrive_expect_tx(bar_full, (uint32_t)__popc(valid) * NBW * 16u);
+    __syncwarp();
+    if (lane < 8 && slot >= 0)
+        bulk_g2s(smem_u32(stage + C::VA_OFF + (i8 * C::SA + 7 - i8) * 2), a.hh_v + slot * NBW * 2, NBW * 16u, bar_full);
+    // VB[7 - i + r][i]: lanes run along i, 4 rows per instruction
+    if (slot >= 0) {
+#pragma unroll
+        for (int t = 0; t < NBW / 4; ++t) {
+            const int rr = t * 4 + (lane >> 3);
+            cp_async16(smem_u32(stage + C::VB_OFF + ((7 - i8 + rr) * C::SB + i8) * 2), a.hh_v + (slot * NBW + rr) * 2, 16u);
+        }
+    }
+    // -T: 64 elements
+    cp_async16(smem_u32(stage + C::TN_OFF + 2 * lane), a.tn + id * 128 + 2 * lane, 16u);
+    cp_async16(smem_u32(stage + C::TN_OFF + 64 + 2 * lane), a.tn + id * 128 + 64 + 2 * lane, 16u);
+    cp_async_mbar_arrive_noinc_wy(bar_full);
+}
+
+// ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column (interleaved in memory, planar in regs) ----
+__device__ __forceinline__ void wyz_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &xr0,
+                                          double &xr1, double &xi0, double &xi1)
+{
+    xr0 = xr1 = xi0 = xi1 = 0.0;
+    if (!colok || row >= a.N) return;
+    const double2 v = *reinterpret_cast<const double2 *>(colp + 2 * row);
+    xr0 = v.x;
+    xi0 = v.y;
+    if (row + 1 < a.N) {
+        const double2 w = *reinterpret_cast<const double2 *>(colp + 2 * row + 2);
+        xr1 = w.x;
+        xi1 = w.y;
+    }
+}
+__device__ __forceinline__ void wyz_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double xr0,
+                                           double xr1, double xi0, double xi1)
+{
+    if (!colok || row >= a.N) return;
+    *reinterpret_cast<double2 *>(colp + 2 * row) = make_double2(xr0, xi0);
+    if (row + 1 < a.N) *reinterpret_cast<double2 *>(colp + 2 * row + 2) = make_double2(xr1, xi1);
+}
+
+// ---- a warp with NG slabs of 8 columns -------------------------------------------------------------------
+template <class C, int NG>
+__device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem, const int warp, const int lane,
+                                            const int nact, const int64_t col0)
+{
+    constexpr int NT = C::NT, NS = C::NS, NBW = C::NBW, LAG = C::LAG;
+    double *ring = reinterpret_cast<double *>(smem);
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + NS * 8;
+    const int gq = lane >> 2, r = lane & 3;
+    const int64_t N = a.N;
+    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t bhi = wy_bhi(N);
+    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t nblocks = wy_nblocks(N, C::LG);
+
+    // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1 (ldq counts complex elements)
+    double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq * 2;
+    const int64_t ldq8 = a.ldq << 4;
+    const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
+
+    int64_t pk = 0, pb = bhi;                           // staging cursor: block it + NS - LAG
+    auto advance = [&]() {
+        if (pb > (pk << (C::LG - 3))) {
+            --pb;
+        } else {
+            ++pk;
+            pb = bhi;
+        }
+    };
+    if (warp == 0) {
+        for (int i = 0; i < NS - LAG; ++i) {
+            if (i < nblocks) wyz_stage<C>(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pk, pb, i, FN1, lane);
+            advance();
+        }
+    } else {
+        for (int i = 0; i < NS - LAG; ++i) advance();
+    }
+
+    double Xr[NG][NT + 1][2], Xi[NG][NT + 1][2];
+    int64_t it = 0;
+    uint32_t duty = 0;
+    for (int64_t k = 0; k < K0; ++k) {
+        const int64_t blo = k << (C::LG - 3);
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+#pragma unroll
+            for (int t = 1; t <= NT; ++t) Xr[g][t][0] = Xr[g][t][1] = Xi[g][t][0] = Xi[g][t][1] = 0.0;
+            wyz_load2(a, cb + g * ldq8, 8 * g < ncolrem, (bhi << 3) + 2 * r, Xr[g][0][0], Xr[g][0][1], Xi[g][0][0],
+                      Xi[g][0][1]);
+        }
+        for (int64_t b = bhi; b >= blo; --b, ++it) {
+            if (duty == (uint32_t)warp) {
+                const int64_t jt = it + NS - LAG;
+                if (jt < nblocks) {
+                    const uint32_t st = (uint32_t)(jt % NS);
+                    if (it >= LAG) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - LAG) / NS) & 1));
+                    wyz_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, jt, FN1, lane);
+                }
+            }
+            advance();
+            duty = (duty + 1 == (uint32_t)nact) ? 0 : duty + 1;
+
+            const uint32_t st = (uint32_t)(it % NS), ph = (uint32_t)((it / NS) & 1);
+            mbar_wait(bar_full + 8 * st, ph);
+            const double *stage = ring + st * C::STAGE_DOUBLES;
+            const double *va = stage + C::VA_OFF + (gq * C::SA + 2 * r) * 2;   // + (8t + e) * 2
+            const double *vb = stage + C::VB_OFF + (gq * C::SB + 2 * r) * 2;   // + 8t * SB * 2 + e * 2
+            const double *tn = stage + C::TN_OFF + (gq * 8 + 2 * r) * 2;       // + e * 2
+
+            // --- D^T = x^T conj(V): A1 = xr Vr, A2 = xi Vi, A3 = xi Vr, A4 = xr Vi
+            double A1[NG][2], A2[NG][2], A3[NG][2], A4[NG][2];
+#pragma unroll
+            for (int g = 0; g < NG; ++g)
+                A1[g][0] = A1[g][1] = A2[g][0] = A2[g][1] = A3[g][0] = A3[g][1] = A4[g][0] = A4[g][1] = 0.0;
+#pragma unroll
+            for (int tt = 0; tt < NT; ++tt) {
+                const int t = (tt + 1) % NT;
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double2 v2 = *reinterpret_cast<const double2 *>(va + (8 * t + e) * 2);
+#pragma unroll
+                    for (int g = 0; g < NG; ++g) {
+                        dmma884(A1[g][0], A1[g][1], Xr[g][t][e], v2.x, A1[g][0], A1[g][1]);
+                        dmma884(A2[g][0], A2[g][1], Xi[g][t][e], v2.y, A2[g][0], A2[g][1]);
+                        dmma884(A3[g][0], A3[g][1], Xi[g][t][e], v2.x, A3[g][0], A3[g][1]);
+                        dmma884(A4[g][0], A4[g][1], Xr[g][t][e], v2.y, A4[g][0], A4[g][1]);
+                    }
+                }
+            }
+            // --- E^T = D^T (-T)^T: Er = Dr TNr - Di TNi, Ei = Dr TNi + Di TNr
+            double Er[NG][2], Ei[NG][2], nEi[NG][2];
+            {
+                const double2 t0 = *reinterpret_cast<const double2 *>(tn);
+                const double2 t1 = *reinterpret_cast<const double2 *>(tn + 2);
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+                    const double dr0 = A1[g][0] + A2[g][0], dr1 = A1[g][1] + A2[g][1];
+                    const double di0 = A3[g][0] - A4[g][0], di1 = A3[g][1] - A4[g][1];
+                    double er0 = 0.0, er1 = 0.0, ei0 = 0.0, ei1 = 0.0;
+                    dmma884(er0, er1, dr0, t0.x, er0, er1);
+                    dmma884(ei0, ei1, dr0, t0.y, ei0, ei1);
+                    dmma884(er0, er1, -di0, t0.y, er0, er1);
+                    dmma884(ei0, ei1, di0, t0.x, ei0, ei1);
+                    dmma884(er0, er1, dr1, t1.x, er0, er1);
+                    dmma884(ei0, ei1, dr1, t1.y, ei0, ei1);
+                    dmma884(er0, er1, -di1, t1.y, er0, er1);
+                    dmma884(ei0, ei1, di1, t1.x, ei0, ei1);
+                    Er[g][0] = er0;
+                    Er[g][1] = er1;
+                    Ei[g][0] = ei0;
+                    Ei[g][1] = ei1;
+                    nEi[g][0] = -ei0;
+                    nEi[g][1] = -ei1;
+                }
+            }
+            // --- x^T += E^T V^T: xr += Er Vr - Ei Vi, xi += Er Vi + Ei Vr; tile t -> registers of t+1
+#pragma unroll
+            for (int t = NT - 1; t >= 0; --t) {
+                const double2 v0 = *reinterpret_cast<const double2 *>(vb + 8 * t * C::SB * 2);
+                const double2 v1 = *reinterpret_cast<const double2 *>(vb + 8 * t * C::SB * 2 + 2);
+#pragma unroll
+                for (int g = 0; g < NG; ++g) {
+                    double m0, m1, n0, n1;
+                    dmma884(m0, m1, Er[g][0], v0.x, Xr[g][t][0], Xr[g][t][1]);
+                    dmma884(n0, n1, Er[g][0], v0.y, Xi[g][t][0], Xi[g][t][1]);
+                    dmma884(m0, m1, nEi[g][0], v0.y, m0, m1);
+                    dmma884(n0, n1, Ei[g][0], v0.x, n0, n1);
+                    dmma884(m0, m1, Er[g][1], v1.x, m0, m1);
+                    dmma884(n0, n1, Er[g][1], v1.y, n0, n1);
+                    dmma884(Xr[g][t + 1][0], Xr[g][t + 1][1], nEi[g][1], v1.y, m0, m1);
+                    dmma884(Xi[g][t + 1][0], Xi[g][t + 1][1], Ei[g][1], v1.x, n0, n1);
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(bar_empty + 8 * st);
+#pragma unroll
+            for (int g = 0; g < NG; ++g) {
+                wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
+                           Xi[g][NT][0], Xi[g][NT][1]);
+                if (b > blo)
+                    wyz_load2(a, cb + g * ldq8, 8 * g < ncolrem, ((b - 1) << 3) + 2 * r, Xr[g][0][0], Xr[g][0][1],
+                              Xi[g][0][0], Xi[g][0][1]);
+            }
+        }
+#pragma unroll
+        for (int g = 0; g < NG; ++g)
+#pragma unroll
+            for (int t = 1; t < NT; ++t)
+                wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, Xr[g][t][0], Xr[g][t][1],
+                           Xi[g][t][0], Xi[g][t][1]);
+    }
+}
+
+// ---- the kernel --------------------------------------------------------------------------------------------
+template <int NBW>
+__global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
+{
+    using C = WyzCfg<NBW>;
+    constexpr int NS = C::NS, NW = C::NW, NGMAX = C::NGMAX;
+    extern __shared__ __align__(128) unsigned char smem[];
+    double *ring = reinterpret_cast<double *>(smem);
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + NS * 8;
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t nslab = (a.nev + 7) >> 3;
+    const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
+    const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
+    const int nact = nmine < NW ? nmine : NW;
+    const int base = nmine / NW, extra = nmine % NW;
+    const int ng = base + (warp < extra ? 1 : 0);
+    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
+
+    for (int i = threadIdx.x; i < C::OFF_BAR / 8; i += blockDim.x) ring[i] = 0.0;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (threadIdx.x == 0) {
+        for (int i = 0; i < NS; ++i) {
+            mbar_init(bar_full + 8 * i, 33);           // 32 cp.async arrivals + the expect_tx arrival
+            mbar_init(bar_empty + 8 * i, (uint32_t)nact);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (ng == 0) return;
+
+    const int64_t col0 = wslab0 << 3;
+    if (NGMAX >= 2 && ng == 2)
+        wyz_consume<C, (NGMAX >= 2 ? 2 : 1)>(a, smem, warp, lane, nact, col0);
+    else
+        wyz_consume<C, 1>(a, smem, warp, lane, nact, col0);
+}
+
+template <int NBW>
+size_t wyz_scratch_bytes(int64_t N)
+{
+    return (size_t)wy_nblocks(N, WyzCfg<NBW>::LG) * 128 * sizeof(double);
+}
+
+template <int NBW>
+cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+                       int nsm, double *tn_scratch, cudaStream_t st)
+{
+    using C = WyzCfg<NBW>;
+    auto kern = bt_wyz_kernel<NBW>;
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int64_t K0 = wy_nchains(N, C::LG);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
+    wyz_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const int64_t nslab = (nev + 7) >> 3;
+    const int64_t per_cta = (int64_t)C::NW * C::NGMAX;
+    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
+    int64_t grid = nsm * waves;
+    if (grid > nslab) grid = nslab;
+    WyArgs a;
+    a.N = N;
+    a.nev = nev;
+    a.ldq = ldq;
+    a.hh_v = hh_v;
+    a.hh_tau = hh_tau;
+    a.q = q;
+    a.tn = tn_scratch;
+    a.align16 = 1;
+    kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace elpa2bt

@@ -1,6 +1,7 @@
 // elpa2_bt.cu -- C-ABI entry points of include/elpa2_bt.h: argument validation, launch planning,
-// host-buffer wrapper.  All arithmetic of the path is in the kernels (bt_wy.cuh: real, DMMA
-// compact-WY; bt_shift.cuh: complex, register window; bt_simple.cuh: plain A/B baseline).
+// host-buffer wrapper.  All arithmetic of the path is in the kernels (bt_wy.cuh / bt_wyz.cuh: the
+// default, compact-WY on the FP64 tensor cores, real / complex; bt_shift.cuh: variant 2, one
+// reflector at a time in a register window, DFMA; bt_simple.cuh: variant 1, plain A/B baseline).
 // No torch types, no CPU fallback.
 #include "../../include/elpa2_bt.h"
 
@@ -11,6 +12,7 @@
 #include "bt_shift.cuh"
 #include "bt_simple.cuh"
 #include "bt_wy.cuh"
+#include "bt_wyz.cuh"
 
 using namespace elpa2bt;
 
@@ -118,6 +120,20 @@ cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_
     return e != cudaSuccess ? e : e2;
 }
 
+template <int NBW>
+cudaError_t run_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+                    cudaStream_t st)
+{
+    cudaError_t e;
+    cudaMemPool_t pool = scratch_pool(&e);
+    if (!pool) return e;
+    void *tn = nullptr;
+    if ((e = cudaMallocFromPoolAsync(&tn, wyz_scratch_bytes<NBW>(N), pool, st)) != cudaSuccess) return e;
+    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), (double *)tn, st);
+    const cudaError_t e2 = cudaFreeAsync(tn, st);
+    return e != cudaSuccess ? e : e2;
+}
+
 template <bool CPLX>
 int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
         void *stream)
@@ -143,7 +159,14 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
         const unsigned grid = (unsigned)((nev + 127) / 128);
         bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
         e = cudaGetLastError();
-    } else if (g_variant == 0 && !CPLX) {
+    } else if (g_variant == 0 && CPLX) {
+        switch (nbw) {
+        case 32: e = run_wyz<32>(N, nev, hh_v, hh_tau, q, ldq, st); break;
+        case 64: e = run_wyz<64>(N, nev, hh_v, hh_tau, q, ldq, st); break;
+        default: e = run_wyz<128>(N, nev, hh_v, hh_tau, q, ldq, st); break;
+        }
+        nlaunch = 2;
+    } else if (g_variant == 0) {
         const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
         switch (nbw) {
         case 32: e = run_wy<32>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;

@@ -94,6 +94,14 @@ def test_simple_variant_matches_oracle(cplx):
     _check(300, 128, 21, cplx, variant=1)
 
 
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_register_window_variant_matches_oracle(nbw, cplx):
+    # variant 2: one reflector at a time (DFMA), the A/B partner of the default compact-WY path
+    _check(3 * nbw + 5, nbw, 100, cplx, variant=2)
+    _check(2 * nbw + 9, nbw, 19, cplx, ldq=2 * nbw + 9 + 3, variant=2)
+
+
 def test_degenerate_no_work():
     for N, nev in ((0, 5), (1, 5), (40, 0)):
         x = np.zeros((N, nev), order="F")
@@ -123,7 +131,7 @@ def test_host_entry_point(cplx):
     y = np.array(x, order="F", copy=True)
     binding.trans_ev_tridi_to_band_host(N, nbw, hh_v, hh_tau, y)
     assert np.abs(y - want).max() <= TOL * np.abs(x).max()
-    assert binding.last_launch_count() == (1 if cplx else 2)     # real: prepass + main kernel
+    assert binding.last_launch_count() == 2     # T-factor prepass + main kernel
 
 
 def test_launch_on_side_stream():
