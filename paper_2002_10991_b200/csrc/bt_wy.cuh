@@ -43,6 +43,7 @@ struct WyCfg {
     static constexpr int NW = 8;                      // warps per CTA
     static constexpr int NGMAX = (NBW <= 64) ? 4 : 2; // most 8-column slabs per warp
     static constexpr int NS = 8;                      // ring stages
+    static constexpr int LGNS = 3;
     static constexpr int LAG = 4;                     // staging waits for the block LAG iterations back
     static constexpr int VA_OFF = 0;                  // VA[i][w], row stride W
     static constexpr int VB_OFF = 8 * W;              // VB[w][i], row stride 8
@@ -59,7 +60,9 @@ struct WyArgs {
     const double *hh_tau;  // G
     double *q;
     double *tn;            // scratch: 64 doubles (-T, row-major) per block, in consumption order
+    uint32_t *prog;        // chain-parallel mode: prog[slab * K0 + k] = blocks of chain k finished (zeroed per call)
     int align16;           // q base and ldq*8 are 16-byte aligned
+    int P;                 // warps per slab (1, 2 or 4), each on its own chains k = p, p+P, ...
 };
 
 // ---- block enumeration ----------------------------------------------------------------------------
@@ -177,7 +180,25 @@ __device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_
     cp_async_mbar_arrive_noinc_wy(bar_full);
 }
 
+// ---- chain-parallel hand-over (P > 1) ------------------------------------------------------------------
+// Chain k+1 may load tile 0 of its block b once chain k has retired rows 8b .. 8b+7, i.e. finished
+// block b - nbw/8 (R5: chain k+1 needs only what chain k has made final).  The writer publishes
+// "blocks finished" with a release store after its tile stores; the reader polls with acquire loads.
+// All warps of a slab sit in one CTA, so CTA scope is enough (at GPU scope the release compiles to
+// MEMBAR.GPU + ERRBAR and costs 27 % of the kernel); q is still read with ld.global.cg.
+__device__ __forceinline__ void prog_publish(uint32_t *p, uint32_t v)
+{
+    asm volatile("st.release.cta.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint32_t prog_read(const uint32_t *p)
+{
+    uint32_t v;
+    asm volatile("ld.acquire.cta.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+
 // ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column ------------------------------------------
+template <bool CG = false>
 __device__ __forceinline__ void wy_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &x0,
                                          double &x1)
 {
@@ -185,12 +206,13 @@ __device__ __forceinline__ void wy_load2(const WyArgs &a, const double *colp, bo
     x1 = 0.0;
     if (!colok || row >= a.N) return;
     if (a.align16 && row + 1 < a.N) {
-        const double2 v = *reinterpret_cast<const double2 *>(colp + row);
+        const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + row))
+                             : *reinterpret_cast<const double2 *>(colp + row);
         x0 = v.x;
         x1 = v.y;
     } else {
-        x0 = colp[row];
-        if (row + 1 < a.N) x1 = colp[row + 1];
+        x0 = CG ? __ldcg(colp + row) : colp[row];
+        if (row + 1 < a.N) x1 = CG ? __ldcg(colp + row + 1) : colp[row + 1];
     }
 }
 __device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double x0, double x1)
@@ -205,73 +227,96 @@ __device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool co
 }
 
 // ---- a warp with NG slabs of 8 columns ---------------------------------------------------------------
-template <class C, int NG>
-__device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int warp, const int lane,
-                                           const int nact, const int64_t col0)
+// CP = false: the 8 warps of a CTA share one ring and walk every chain (grp = 0, member = warp).
+// CP = true (NG = 1): a.P warps share a slab; warp (grp, member) walks chains grp, grp+P, .. of slab
+// `slab`; the warps with the same grp share ring grp (NS/P stages) and are its `nmem` members.
+template <class C, int NG, bool CP>
+__device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int lane, const int grp,
+                                           const int member, const int nmem, const int64_t col0, const int64_t slab)
 {
-    constexpr int NT = C::NT, W = C::W, NS = C::NS, NBW = C::NBW, LAG = C::LAG;
+    constexpr int NT = C::NT, W = C::W, NBW = C::NBW;
     constexpr int NACC = (NG >= 3) ? 1 : 2;          // dot-product accumulator sets per slab
-    double *ring = reinterpret_cast<double *>(smem);
-    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
-    const uint32_t bar_empty = bar_full + NS * 8;
+    const int P = CP ? a.P : 1;
+    const int lgs = CP ? (P == 2 ? C::LGNS - 1 : C::LGNS - 2) : C::LGNS;   // log2(stages of this ring)
+    const int NSP = 1 << lgs, LAG = NSP >> 1;
+    double *ring = reinterpret_cast<double *>(smem) + (size_t)grp * NSP * C::STAGE_DOUBLES;
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR) + 8 * grp * NSP;
+    const uint32_t bar_empty = bar_full + C::NS * 8;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::LG);
     const int64_t bhi = wy_bhi(N);
     const int64_t FN1 = hh_F(N - 1, C::LG);
-    const int64_t nblocks = wy_nblocks(N, C::LG);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq;
     const int64_t ldq8 = a.ldq << 3;
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
 
-    // staging cursor: block it + NS - LAG
-    int64_t pk = 0, pb = bhi;
+    // staging cursor: block it + NSP - LAG of this ring's sequence
+    int64_t pk = grp, pb = bhi;
     auto advance = [&]() {
         if (pb > (pk << (C::LG - 3))) {
             --pb;
         } else {
-            ++pk;
+            pk += P;
             pb = bhi;
         }
     };
-    // prologue: blocks 0 .. NS-LAG-1 go into fresh stages
-    if (warp == 0) {
-        for (int i = 0; i < NS - LAG; ++i) {
-            if (i < nblocks) wy_stage<C>(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pk, pb, i, FN1, lane);
-            advance();
-        }
-    } else {
-        for (int i = 0; i < NS - LAG; ++i) advance();
+    auto stage_cursor = [&](uint32_t st) {
+        wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::LG, pk) + (bhi - pb), FN1,
+                    lane);
+    };
+    // prologue: blocks 0 .. NSP-LAG-1 go into fresh stages
+    for (int i = 0; i < NSP - LAG; ++i) {
+        if (member == 0 && pk < K0) stage_cursor((uint32_t)i);
+        advance();
     }
 
-    double X[NG][NT + 1][2];
-    int64_t it = 0;
-    uint32_t duty = 0;
-    for (int64_t k = 0; k < K0; ++k) {
+    // tile 0 is loaded one block ahead of its block; two blocks ahead when a warp has so few slabs
+    // that a block is shorter than a DRAM round trip (Pf holds the tile of the block after next)
+    constexpr bool PF2 = (NG <= 2);
+    // X[g][t], t = 1 .. NT-1: tiles of the window above tile 0; X[g][NT]: the tile that retires.
+    // Tile 0 lives in TA / TB: with PF2 the blocks alternate between the two buffers (a buffer is
+    // refilled with the tile of the block after next as soon as its block is done, so no register
+    // copy ever waits for a load); otherwise every block uses TA.
+    double X[NG][NT + 1][2], TA[NG][2], TB[NG][2];
+    uint32_t it = 0;                   // blocks consumed from this ring
+    int duty = 0;
+    for (int64_t k = grp; k < K0; k += P) {
         const int64_t blo = k << (C::LG - 3);
+        // chain-parallel hand-over: chain k-1 of this slab is walked by another warp of the CTA
+        const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
+        uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
+        uint32_t known = 0;
+        auto wait_prev = [&](int64_t b) {          // before loading tile 0 of block b
+            if (CP && prev) {
+                const uint32_t need = (uint32_t)(bhi - b + NBW / 8 + 1);
+                while (known < need) known = prog_read(prev);
+            }
+        };
+        auto load_tile0 = [&](int64_t b, double (&T0)[NG][2]) {
+            if (b < blo) return;
+            wait_prev(b);
 #pragma unroll
-        for (int g = 0; g < NG; ++g) {
-#pragma unroll
-            for (int t = 1; t <= NT; ++t) X[g][t][0] = X[g][t][1] = 0.0;
-            wy_load2(a, cb + g * ldq8, 8 * g < ncolrem, (bhi << 3) + 2 * r, X[g][0][0], X[g][0][1]);
-        }
-        for (int64_t b = bhi; b >= blo; --b, ++it) {
-            // --- staging duty: block it+NS-LAG goes into the stage that block it-LAG used; the warp
-            //     on duty only waits if some warp is still LAG blocks behind it
-            if (duty == (uint32_t)warp) {
-                const int64_t jt = it + NS - LAG;
-                if (jt < nblocks) {
-                    const uint32_t st = (uint32_t)(jt % NS);
-                    if (it >= LAG) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - LAG) / NS) & 1));
-                    wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, jt, FN1, lane);
+            for (int g = 0; g < NG; ++g)
+                wy_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1]);
+        };
+        // one block: T0 = its tile 0 on entry, tile 0 of block b - (PF2 ? 2 : 1) on exit
+        auto do_block = [&](const int64_t b, double (&T0)[NG][2]) {
+            // --- staging duty: block it+NSP-LAG goes into the stage that block it-LAG used; the warp
+            //     on duty only waits if some member is still LAG blocks behind it
+            if (duty == member) {
+                if (pk < K0) {
+                    const uint32_t st = (it + NSP - LAG) & (NSP - 1);
+                    if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
+                    stage_cursor(st);
                 }
             }
             advance();
-            duty = (duty + 1 == (uint32_t)nact) ? 0 : duty + 1;
+            duty = (duty + 1 == nmem) ? 0 : duty + 1;
 
-            const uint32_t st = (uint32_t)(it % NS), ph = (uint32_t)((it / NS) & 1);
+            const uint32_t st = it & (NSP - 1), ph = (it >> lgs) & 1;
             mbar_wait(bar_full + 8 * st, ph);
             const double *stage = ring + st * C::STAGE_DOUBLES;
             const double *va = stage + C::VA_OFF + gq * W + 2 * r;
@@ -290,10 +335,11 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
                 const double2 v2 = *reinterpret_cast<const double2 *>(va + 8 * t);
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
-                    dmma884(D[g][0][0], D[g][0][1], X[g][t][0], v2.x, D[g][0][0], D[g][0][1]);
+                    dmma884(D[g][0][0], D[g][0][1], t ? X[g][t][0] : T0[g][0], v2.x, D[g][0][0], D[g][0][1]);
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
-                    dmma884(D[g][NACC - 1][0], D[g][NACC - 1][1], X[g][t][1], v2.y, D[g][NACC - 1][0], D[g][NACC - 1][1]);
+                    dmma884(D[g][NACC - 1][0], D[g][NACC - 1][1], t ? X[g][t][1] : T0[g][1], v2.y, D[g][NACC - 1][0],
+                            D[g][NACC - 1][1]);
             }
             // --- E^T = D^T (-T)^T
             double E[NG][2];
@@ -318,19 +364,40 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
 #pragma unroll
                 for (int g = 0; g < NG; ++g) {
                     double m0, m1;
-                    dmma884(m0, m1, E[g][0], v2.x, X[g][t][0], X[g][t][1]);
+                    dmma884(m0, m1, E[g][0], v2.x, t ? X[g][t][0] : T0[g][0], t ? X[g][t][1] : T0[g][1]);
                     dmma884(X[g][t + 1][0], X[g][t + 1][1], E[g][1], v2.y, m0, m1);
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * st);
-            // --- tile NT-1 retires (rows 8b + nbw ..), tile 0 of the next block comes in
-#pragma unroll
-            for (int g = 0; g < NG; ++g) {
-                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
-                if (b > blo)
-                    wy_load2(a, cb + g * ldq8, 8 * g < ncolrem, ((b - 1) << 3) + 2 * r, X[g][0][0], X[g][0][1]);
+            if (lane == 0) {
+                mbar_arrive(bar_empty + 8 * st);
+                // the stores of the blocks before this one have long been performed: publishing them
+                // here keeps the release fence off the critical path (costs one block of extra lag)
+                if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
             }
+            // --- tile NT-1 retires (rows 8b + nbw ..), the buffer of tile 0 is refilled
+#pragma unroll
+            for (int g = 0; g < NG; ++g)
+                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
+            load_tile0(b - (PF2 ? 2 : 1), T0);
+            ++it;
+        };
+
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+#pragma unroll
+            for (int t = 1; t <= NT; ++t) X[g][t][0] = X[g][t][1] = 0.0;
+            TA[g][0] = TA[g][1] = TB[g][0] = TB[g][1] = 0.0;
+        }
+        load_tile0(bhi, TA);
+        if (PF2) {
+            load_tile0(bhi - 1, TB);
+            for (int64_t b = bhi; b >= blo; b -= 2) {
+                do_block(b, TA);
+                if (b - 1 >= blo) do_block(b - 1, TB);
+            }
+        } else {
+            for (int64_t b = bhi; b >= blo; --b) do_block(b, TA);
         }
         // --- chain end: tiles 1 .. NT-1 hold rows 8 blo + 8 (t-1) + 2r + {0,1}
 #pragma unroll
@@ -338,13 +405,18 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
 #pragma unroll
             for (int t = 1; t < NT; ++t)
                 wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
+        if (CP) {
+            __syncwarp();
+            if (lane == 0) prog_publish(mine, (uint32_t)(bhi - blo + 1));
+        }
     }
 }
 
 // ---- the kernel ----------------------------------------------------------------------------------------
-// grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid) (at most NW*NGMAX of them); warp w takes
-// n/NW of those, +1 for the first n%NW warps (warps w and w+4 share a sub-partition, so the extras
-// land on different sub-partitions first).
+// grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid).
+//  P = 1: at most NW*NGMAX slabs per CTA; warp w takes n/NW of them, +1 for the first n%NW warps
+//         (warps w and w+4 share a sub-partition, so the extras land on different sub-partitions first).
+//  P > 1 (few slabs): at most NW/P slabs per CTA; warp w works on slab w/P, chains (w%P) + m P.
 template <int NBW>
 __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
 {
@@ -359,10 +431,7 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
     const int64_t nslab = (a.nev + 7) >> 3;
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
-    const int nact = nmine < NW ? nmine : NW;
-    const int base = nmine / NW, extra = nmine % NW;
-    const int ng = base + (warp < extra ? 1 : 0);
-    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
+    const int nact = nmine < NW ? nmine : NW;          // members of a ring (P = 1: active warps)
 
     // the ring starts as zeros: the skew padding of VA / VB is never written by the copies, and
     // positions of reflectors outside a chain keep finite values (their row and column of T are 0)
@@ -375,30 +444,55 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
         mbar_fence_init();
     }
     __syncthreads();
-    if (ng == 0) return;
 
+    if (a.P > 1) {
+        const int grp = warp % a.P, member = warp / a.P;
+        if (member >= nmine) return;
+        wy_consume<C, 1, true>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
+        return;
+    }
+    const int base = nmine / NW, extra = nmine % NW;
+    const int ng = base + (warp < extra ? 1 : 0);
+    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
+    if (ng == 0) return;
     const int64_t col0 = wslab0 << 3;
     if (NGMAX >= 4 && ng == 4)
-        wy_consume<C, (NGMAX >= 4 ? 4 : 1)>(a, smem, warp, lane, nact, col0);
+        wy_consume<C, (NGMAX >= 4 ? 4 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (NGMAX >= 3 && ng == 3)
-        wy_consume<C, (NGMAX >= 3 ? 3 : 1)>(a, smem, warp, lane, nact, col0);
+        wy_consume<C, (NGMAX >= 3 ? 3 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (ng == 2)
-        wy_consume<C, 2>(a, smem, warp, lane, nact, col0);
+        wy_consume<C, 2, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else
-        wy_consume<C, 1>(a, smem, warp, lane, nact, col0);
+        wy_consume<C, 1, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
 }
 
 // ---- host side -----------------------------------------------------------------------------------------
-// bytes of -T scratch the two kernels share
+// warps per slab: with fewer slabs than warp slots, P warps share a slab on different chains
+inline int wy_pick_P(int64_t nslab, int64_t K0, int nsm, int nw, int maxP)
+{
+    const int64_t grid = nslab < nsm ? nslab : nsm;
+    const int64_t spc = (nslab + grid - 1) / grid;     // most slabs per CTA when the grid is one wave
+    int P = 1;
+    while (2 * P <= maxP && spc * 2 * P <= nw && 4 * P <= K0) P *= 2;
+    return nslab <= (int64_t)nsm * nw ? P : 1;
+}
+
+// bytes of scratch the two kernels share: -T factors, then the chain-progress counters
 template <int NBW>
-size_t wy_scratch_bytes(int64_t N)
+size_t wy_tn_bytes(int64_t N)
 {
     return (size_t)wy_nblocks(N, WyCfg<NBW>::LG) * 64 * sizeof(double);
+}
+template <int NBW>
+size_t wy_scratch_bytes(int64_t N, int64_t nev)
+{
+    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, WyCfg<NBW>::LG) * sizeof(uint32_t);
+    return wy_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
 template <int NBW>
 cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                      int align16, int nsm, double *tn_scratch, cudaStream_t st, int *launches)
+                      int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0)
 {
     using C = WyCfg<NBW>;
     auto kern = bt_wy_kernel<NBW>;
@@ -409,12 +503,20 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
         attr_done = true;
     }
     const int64_t K0 = wy_nchains(N, C::LG);
-    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
-    wy_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
-    cudaError_t e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
     const int64_t nslab = (nev + 7) >> 3;
-    const int64_t per_cta = (int64_t)C::NW * C::NGMAX;
+    double *tn = (double *)scratch;
+    uint32_t *prog = (uint32_t *)((char *)scratch + wy_tn_bytes<NBW>(N));
+    const int P = force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 4);
+    cudaError_t e;
+    if (P > 1) {
+        e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
+        if (e != cudaSuccess) return e;
+    }
+    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
+    wy_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
     const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
     int64_t grid = nsm * waves;                       // a multiple of the SM count ...
     if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that
@@ -425,10 +527,11 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     a.hh_v = hh_v;
     a.hh_tau = hh_tau;
     a.q = q;
-    a.tn = tn_scratch;
+    a.tn = tn;
+    a.prog = prog;
     a.align16 = align16;
+    a.P = P;
     kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
-    if (launches) *launches = 2;
     return cudaGetLastError();
 }
 

@@ -392,7 +392,9 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
     a.hh_tau = hh_tau;
     a.q = q;
     a.tn = tn_scratch;
+    a.prog = nullptr;
     a.align16 = 1;
+    a.P = 1;
     kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
     return cudaGetLastError();
 }

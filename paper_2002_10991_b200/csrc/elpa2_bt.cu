@@ -114,8 +114,8 @@ cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
-    if ((e = cudaMallocFromPoolAsync(&tn, wy_scratch_bytes<NBW>(N), pool, st)) != cudaSuccess) return e;
-    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), (double *)tn, st, nullptr);
+    if ((e = cudaMallocFromPoolAsync(&tn, wy_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
+    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), tn, st);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
