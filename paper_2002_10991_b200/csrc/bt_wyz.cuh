@@ -24,6 +24,7 @@ struct WyzCfg {
     static constexpr int NW = 8;                      // warps per CTA
     static constexpr int NGMAX = (NBW <= 64) ? 2 : 1; // most 8-column slabs per warp
     static constexpr int NS = (NBW <= 64) ? 8 : 4;    // ring stages
+    static constexpr int LGNS = (NBW <= 64) ? 3 : 2;
     static constexpr int LAG = NS / 2;                // staging waits for the block LAG iterations back
     // element = 2 doubles.  Row strides padded by one element: rows gq and gq+1 of a quarter-warp
     // then differ by 4 banks (W*4 and 8*4 words are multiples of 32)
@@ -141,16 +142,19 @@ __device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32
 }
 
 // ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column (interleaved in memory, planar in regs) ----
+template <bool CG = false>
 __device__ __forceinline__ void wyz_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &xr0,
                                           double &xr1, double &xi0, double &xi1)
 {
     xr0 = xr1 = xi0 = xi1 = 0.0;
     if (!colok || row >= a.N) return;
-    const double2 v = *reinterpret_cast<const double2 *>(colp + 2 * row);
+    const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row))
+                         : *reinterpret_cast<const double2 *>(colp + 2 * row);
     xr0 = v.x;
     xi0 = v.y;
     if (row + 1 < a.N) {
-        const double2 w = *reinterpret_cast<const double2 *>(colp + 2 * row + 2);
+        const double2 w = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row + 2))
+                             : *reinterpret_cast<const double2 *>(colp + 2 * row + 2);
         xr1 = w.x;
         xi1 = w.y;
     }
@@ -164,69 +168,82 @@ __device__ __forceinline__ void wyz_store2(const WyArgs &a, double *colp, bool c
 }
 
 // ---- a warp with NG slabs of 8 columns -------------------------------------------------------------------
-template <class C, int NG>
-__device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem, const int warp, const int lane,
-                                            const int nact, const int64_t col0)
+// Same structure as wy_consume (bt_wy.cuh): CP = chain-parallel mode (a.P warps per slab, NG = 1).
+template <class C, int NG, bool CP>
+__device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem, const int lane, const int grp,
+                                            const int member, const int nmem, const int64_t col0, const int64_t slab)
 {
-    constexpr int NT = C::NT, NS = C::NS, NBW = C::NBW, LAG = C::LAG;
-    double *ring = reinterpret_cast<double *>(smem);
-    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
-    const uint32_t bar_empty = bar_full + NS * 8;
+    constexpr int NT = C::NT, NBW = C::NBW;
+    const int P = CP ? a.P : 1;
+    const int lgs = CP ? C::LGNS - 1 : C::LGNS;        // P = 2 is the only chain-parallel width here
+    const int NSP = 1 << lgs, LAG = NSP >> 1;
+    double *ring = reinterpret_cast<double *>(smem) + (size_t)grp * NSP * C::STAGE_DOUBLES;
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR) + 8 * grp * NSP;
+    const uint32_t bar_empty = bar_full + C::NS * 8;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::LG);
     const int64_t bhi = wy_bhi(N);
     const int64_t FN1 = hh_F(N - 1, C::LG);
-    const int64_t nblocks = wy_nblocks(N, C::LG);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1 (ldq counts complex elements)
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq * 2;
     const int64_t ldq8 = a.ldq << 4;
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
 
-    int64_t pk = 0, pb = bhi;                           // staging cursor: block it + NS - LAG
+    int64_t pk = grp, pb = bhi;                         // staging cursor: block it + NSP - LAG of this ring
     auto advance = [&]() {
         if (pb > (pk << (C::LG - 3))) {
             --pb;
         } else {
-            ++pk;
+            pk += P;
             pb = bhi;
         }
     };
-    if (warp == 0) {
-        for (int i = 0; i < NS - LAG; ++i) {
-            if (i < nblocks) wyz_stage<C>(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pk, pb, i, FN1, lane);
-            advance();
-        }
-    } else {
-        for (int i = 0; i < NS - LAG; ++i) advance();
+    auto stage_cursor = [&](uint32_t st) {
+        wyz_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::LG, pk) + (bhi - pb), FN1,
+                     lane);
+    };
+    for (int i = 0; i < NSP - LAG; ++i) {
+        if (member == 0 && pk < K0) stage_cursor((uint32_t)i);
+        advance();
     }
 
-    double Xr[NG][NT + 1][2], Xi[NG][NT + 1][2];
-    int64_t it = 0;
-    uint32_t duty = 0;
-    for (int64_t k = 0; k < K0; ++k) {
+    // tile 0 alternates between TA and TB (refilled two blocks ahead, bt_wy.cuh); [..][0..1] = real
+    // parts of rows 2r, 2r+1, [..][2..3] = imaginary parts
+    double Xr[NG][NT + 1][2], Xi[NG][NT + 1][2], TA[NG][4], TB[NG][4];
+    uint32_t it = 0;
+    int duty = 0;
+    for (int64_t k = grp; k < K0; k += P) {
         const int64_t blo = k << (C::LG - 3);
+        const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
+        uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
+        uint32_t known = 0;
+        auto wait_prev = [&](int64_t b) {
+            if (CP && prev) {
+                const uint32_t need = (uint32_t)(bhi - b + NBW / 8 + 1);
+                while (known < need) known = prog_read(prev);
+            }
+        };
+        auto load_tile0 = [&](int64_t b, double (&T0)[NG][4]) {
+            if (b < blo) return;
+            wait_prev(b);
 #pragma unroll
-        for (int g = 0; g < NG; ++g) {
-#pragma unroll
-            for (int t = 1; t <= NT; ++t) Xr[g][t][0] = Xr[g][t][1] = Xi[g][t][0] = Xi[g][t][1] = 0.0;
-            wyz_load2(a, cb + g * ldq8, 8 * g < ncolrem, (bhi << 3) + 2 * r, Xr[g][0][0], Xr[g][0][1], Xi[g][0][0],
-                      Xi[g][0][1]);
-        }
-        for (int64_t b = bhi; b >= blo; --b, ++it) {
-            if (duty == (uint32_t)warp) {
-                const int64_t jt = it + NS - LAG;
-                if (jt < nblocks) {
-                    const uint32_t st = (uint32_t)(jt % NS);
-                    if (it >= LAG) mbar_wait(bar_empty + 8 * st, (uint32_t)(((it - LAG) / NS) & 1));
-                    wyz_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, jt, FN1, lane);
+            for (int g = 0; g < NG; ++g)
+                wyz_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1], T0[g][2], T0[g][3]);
+        };
+        auto do_block = [&](const int64_t b, double (&T0)[NG][4]) {
+            if (duty == member) {
+                if (pk < K0) {
+                    const uint32_t st = (it + NSP - LAG) & (NSP - 1);
+                    if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
+                    stage_cursor(st);
                 }
             }
             advance();
-            duty = (duty + 1 == (uint32_t)nact) ? 0 : duty + 1;
+            duty = (duty + 1 == nmem) ? 0 : duty + 1;
 
-            const uint32_t st = (uint32_t)(it % NS), ph = (uint32_t)((it / NS) & 1);
+            const uint32_t st = it & (NSP - 1), ph = (it >> lgs) & 1;
             mbar_wait(bar_full + 8 * st, ph);
             const double *stage = ring + st * C::STAGE_DOUBLES;
             const double *va = stage + C::VA_OFF + (gq * C::SA + 2 * r) * 2;   // + (8t + e) * 2
@@ -246,10 +263,11 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                     const double2 v2 = *reinterpret_cast<const double2 *>(va + (8 * t + e) * 2);
 #pragma unroll
                     for (int g = 0; g < NG; ++g) {
-                        dmma884(A1[g][0], A1[g][1], Xr[g][t][e], v2.x, A1[g][0], A1[g][1]);
-                        dmma884(A2[g][0], A2[g][1], Xi[g][t][e], v2.y, A2[g][0], A2[g][1]);
-                        dmma884(A3[g][0], A3[g][1], Xi[g][t][e], v2.x, A3[g][0], A3[g][1]);
-                        dmma884(A4[g][0], A4[g][1], Xr[g][t][e], v2.y, A4[g][0], A4[g][1]);
+                        const double xr = t ? Xr[g][t][e] : T0[g][e], xi = t ? Xi[g][t][e] : T0[g][2 + e];
+                        dmma884(A1[g][0], A1[g][1], xr, v2.x, A1[g][0], A1[g][1]);
+                        dmma884(A2[g][0], A2[g][1], xi, v2.y, A2[g][0], A2[g][1]);
+                        dmma884(A3[g][0], A3[g][1], xi, v2.x, A3[g][0], A3[g][1]);
+                        dmma884(A4[g][0], A4[g][1], xr, v2.y, A4[g][0], A4[g][1]);
                     }
                 }
             }
@@ -287,8 +305,8 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
 #pragma unroll
                 for (int g = 0; g < NG; ++g) {
                     double m0, m1, n0, n1;
-                    dmma884(m0, m1, Er[g][0], v0.x, Xr[g][t][0], Xr[g][t][1]);
-                    dmma884(n0, n1, Er[g][0], v0.y, Xi[g][t][0], Xi[g][t][1]);
+                    dmma884(m0, m1, Er[g][0], v0.x, t ? Xr[g][t][0] : T0[g][0], t ? Xr[g][t][1] : T0[g][1]);
+                    dmma884(n0, n1, Er[g][0], v0.y, t ? Xi[g][t][0] : T0[g][2], t ? Xi[g][t][1] : T0[g][3]);
                     dmma884(m0, m1, nEi[g][0], v0.y, m0, m1);
                     dmma884(n0, n1, Ei[g][0], v0.x, n0, n1);
                     dmma884(m0, m1, Er[g][1], v1.x, m0, m1);
@@ -298,15 +316,30 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                 }
             }
             __syncwarp();
-            if (lane == 0) mbar_arrive(bar_empty + 8 * st);
+            if (lane == 0) {
+                mbar_arrive(bar_empty + 8 * st);
+                if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
+            }
 #pragma unroll
-            for (int g = 0; g < NG; ++g) {
+            for (int g = 0; g < NG; ++g)
                 wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
                            Xi[g][NT][0], Xi[g][NT][1]);
-                if (b > blo)
-                    wyz_load2(a, cb + g * ldq8, 8 * g < ncolrem, ((b - 1) << 3) + 2 * r, Xr[g][0][0], Xr[g][0][1],
-                              Xi[g][0][0], Xi[g][0][1]);
-            }
+            load_tile0(b - 2, T0);
+            ++it;
+        };
+
+#pragma unroll
+        for (int g = 0; g < NG; ++g) {
+#pragma unroll
+            for (int t = 1; t <= NT; ++t) Xr[g][t][0] = Xr[g][t][1] = Xi[g][t][0] = Xi[g][t][1] = 0.0;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) TA[g][i] = TB[g][i] = 0.0;
+        }
+        load_tile0(bhi, TA);
+        load_tile0(bhi - 1, TB);
+        for (int64_t b = bhi; b >= blo; b -= 2) {
+            do_block(b, TA);
+            if (b - 1 >= blo) do_block(b - 1, TB);
         }
 #pragma unroll
         for (int g = 0; g < NG; ++g)
@@ -314,6 +347,10 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             for (int t = 1; t < NT; ++t)
                 wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, Xr[g][t][0], Xr[g][t][1],
                            Xi[g][t][0], Xi[g][t][1]);
+        if (CP) {
+            __syncwarp();
+            if (lane == 0) prog_publish(mine, (uint32_t)(bhi - blo + 1));
+        }
     }
 }
 
@@ -333,9 +370,6 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
     const int nact = nmine < NW ? nmine : NW;
-    const int base = nmine / NW, extra = nmine % NW;
-    const int ng = base + (warp < extra ? 1 : 0);
-    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
 
     for (int i = threadIdx.x; i < C::OFF_BAR / 8; i += blockDim.x) ring[i] = 0.0;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -347,24 +381,39 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
         mbar_fence_init();
     }
     __syncthreads();
-    if (ng == 0) return;
 
+    if (a.P > 1) {
+        const int grp = warp % a.P, member = warp / a.P;
+        if (member >= nmine) return;
+        wyz_consume<C, 1, true>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
+        return;
+    }
+    const int base = nmine / NW, extra = nmine % NW;
+    const int ng = base + (warp < extra ? 1 : 0);
+    const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
+    if (ng == 0) return;
     const int64_t col0 = wslab0 << 3;
     if (NGMAX >= 2 && ng == 2)
-        wyz_consume<C, (NGMAX >= 2 ? 2 : 1)>(a, smem, warp, lane, nact, col0);
+        wyz_consume<C, (NGMAX >= 2 ? 2 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else
-        wyz_consume<C, 1>(a, smem, warp, lane, nact, col0);
+        wyz_consume<C, 1, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
 }
 
 template <int NBW>
-size_t wyz_scratch_bytes(int64_t N)
+size_t wyz_tn_bytes(int64_t N)
 {
     return (size_t)wy_nblocks(N, WyzCfg<NBW>::LG) * 128 * sizeof(double);
+}
+template <int NBW>
+size_t wyz_scratch_bytes(int64_t N, int64_t nev)
+{
+    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, WyzCfg<NBW>::LG) * sizeof(uint32_t);
+    return wyz_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
 template <int NBW>
 cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                       int nsm, double *tn_scratch, cudaStream_t st)
+                       int nsm, void *scratch, cudaStream_t st, int force_P = 0)
 {
     using C = WyzCfg<NBW>;
     auto kern = bt_wyz_kernel<NBW>;
@@ -375,12 +424,20 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
         attr_done = true;
     }
     const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t nslab = (nev + 7) >> 3;
+    double *tn_scratch = (double *)scratch;
+    uint32_t *prog = (uint32_t *)((char *)scratch + wyz_tn_bytes<NBW>(N));
+    const int P = force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 2);
+    cudaError_t e;
+    if (P > 1) {
+        e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
+        if (e != cudaSuccess) return e;
+    }
     const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
     wyz_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
-    cudaError_t e = cudaGetLastError();
+    e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const int64_t nslab = (nev + 7) >> 3;
-    const int64_t per_cta = (int64_t)C::NW * C::NGMAX;
+    const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
     const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
     int64_t grid = nsm * waves;
     if (grid > nslab) grid = nslab;
@@ -392,9 +449,9 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
     a.hh_tau = hh_tau;
     a.q = q;
     a.tn = tn_scratch;
-    a.prog = nullptr;
+    a.prog = prog;
     a.align16 = 1;
-    a.P = 1;
+    a.P = P;
     kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
     return cudaGetLastError();
 }

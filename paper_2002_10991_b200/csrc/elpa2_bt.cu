@@ -128,8 +128,8 @@ cudaError_t run_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
-    if ((e = cudaMallocFromPoolAsync(&tn, wyz_scratch_bytes<NBW>(N), pool, st)) != cudaSuccess) return e;
-    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), (double *)tn, st);
+    if ((e = cudaMallocFromPoolAsync(&tn, wyz_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
+    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), tn, st);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
