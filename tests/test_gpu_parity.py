@@ -88,6 +88,17 @@ def test_many_warps_and_ctas(nbw, cplx):
 
 
 @pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_chain_parallel_mode(nbw, cplx):
+    # few columns and many chains: P = 2 / 4 warps share a slab, each on its own chains, with the
+    # hand-over of retired rows through global memory; ragged N, ragged last slab
+    _check(9 * nbw + 3, nbw, 5, cplx)            # K0 = 10: P = 2, one slab
+    _check(17 * nbw + 1, nbw, 9, cplx)           # K0 = 18: P = 4 (real) / 2 (complex), two slabs
+    _check(16 * nbw, nbw, 200, cplx)             # 25 slabs on 25 CTAs
+    _check(12 * nbw + 7, nbw, 148 * 8 * 3 + 5, cplx)   # 3-4 slabs per CTA: P = 2, ragged tail
+
+
+@pytest.mark.parametrize("cplx", [False, True])
 def test_simple_variant_matches_oracle(cplx):
     _check(150, 32, 37, cplx, variant=1)
     _check(300, 64, 21, cplx, variant=1)
