@@ -45,10 +45,11 @@ struct WyCfg {
     static constexpr int NS = 8;                      // ring stages
     static constexpr int LGNS = 3;
     static constexpr int LAG = 4;                     // staging waits for the block LAG iterations back
-    static constexpr int VA_OFF = 0;                  // VA[i][w], row stride W
-    static constexpr int VB_OFF = 8 * W;              // VB[w][i], row stride 8
-    static constexpr int TN_OFF = 16 * W;             // TN[n][k] = -T[n][k]
-    static constexpr int STAGE_DOUBLES = 16 * W + 64;
+    static constexpr int VA_OFF = 0;                  // VA[i][w] = V, row stride W
+    static constexpr int YB_OFF = 8 * W;              // YB[w][j] = (V (-T))[w][j], row stride 8
+    static constexpr int STAGE_DOUBLES = 16 * W;
+    static constexpr int YBLK = 8 * W;                // doubles of scratch per block (its YB image)
+    static constexpr int PW = (NBW <= 64) ? 8 : 4;    // warps (= blocks) per CTA of the prepass kernel
     static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
     static_assert(W % 16 == 8, "VA row stride must be 8 mod 16 doubles (bank-conflict-free LDS.128)");
@@ -59,7 +60,7 @@ struct WyArgs {
     const double *hh_v;    // G * nbw
     const double *hh_tau;  // G
     double *q;
-    double *tn;            // scratch: 64 doubles (-T, row-major) per block, in consumption order
+    double *tn;            // scratch of the prepass, per block in consumption order (real: the YB image)
     uint32_t *prog;        // chain-parallel mode: prog[slab * K0 + k] = blocks of chain k finished (zeroed per call)
     int align16;           // q base and ldq*8 are 16-byte aligned
     int P;                 // warps per slab (1, 2 or 4), each on its own chains k = p, p+P, ...
@@ -100,22 +101,27 @@ __device__ __forceinline__ void cp_async_mbar_arrive_noinc_wy(uint32_t bar)
     asm volatile("cp.async.mbarrier.arrive.noinc.shared::cta.b64 [%0];" ::"r"(bar) : "memory");
 }
 
-// ---- prepass: -T of every block -------------------------------------------------------------------
-// grid (ceil((bhi+1)/8), K0), 256 threads: warp = one block (k, b).  Lane (gq, r) loads column gq
-// of V at window rows 4c + r, c = 0 .. W/4-1 (both the A and the B fragment of V^T V), the Gram
-// matrix comes out of W/4 DMMAs, then lane l & 7 runs the recurrence for column l of T.
+// ---- prepass: Y = V (-T) of every block ------------------------------------------------------------
+// grid (ceil((bhi+1)/PW), K0), PW warps: warp = one block (k, b).  Lane (gq, r) loads column gq
+// of V at window rows 4c + r, c = 0 .. W/4-1 (both the A and the B fragment of V^T V; also parked in
+// shared memory), the Gram matrix comes out of W/4 DMMAs, lane l & 7 runs the recurrence of R6 for
+// column l of T, and W/4 more DMMAs give Y = V (-T), stored as the YB[w][j] image the main kernel
+// stages with one bulk copy.
 template <int NBW>
-__global__ void __launch_bounds__(256) wy_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
-                                                         const double *__restrict__ hh_tau, double *__restrict__ tn)
+__global__ void __launch_bounds__(WyCfg<NBW>::PW * 32) wy_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
+                                                                         const double *__restrict__ hh_tau,
+                                                                         double *__restrict__ yb)
 {
     using C = WyCfg<NBW>;
-    __shared__ double Sm[8][64];
+    constexpr int W = C::W, SV = W + 2;               // Vs row stride: rows r, r+1 land 4 banks apart
+    __shared__ double Sm[C::PW][64];
+    __shared__ double Vs[C::PW][8 * SV];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t k = blockIdx.y;
     const int64_t bhi = wy_bhi(N);
     const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
-    const int64_t j = (int64_t)blockIdx.x * 8 + warp;
+    const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
     if (j >= nblk) return;
     const int64_t b = bhi - j;
     const int64_t FN1 = hh_F(N - 1, C::LG);
@@ -123,9 +129,10 @@ __global__ void __launch_bounds__(256) wy_prepass_kernel(int64_t N, const double
     const double tau = slot >= 0 ? hh_tau[slot] : 0.0;
     double s0 = 0.0, s1 = 0.0, u0 = 0.0, u1 = 0.0;
 #pragma unroll
-    for (int c = 0; c < C::W / 4; ++c) {
+    for (int c = 0; c < W / 4; ++c) {
         const int rl = 4 * c + r - (7 - gq);
         const double v = (slot >= 0 && rl >= 0 && rl < NBW) ? hh_v[slot * NBW + rl] : 0.0;
+        Vs[warp][gq * SV + 4 * c + r] = v;
         if (c & 1)
             dmma884(u0, u1, v, v, u0, u1);
         else
@@ -145,14 +152,26 @@ __global__ void __launch_bounds__(256) wy_prepass_kernel(int64_t N, const double
         for (int i = 0; i < jj; ++i) acc = fma(Sm[warp][jj * 8 + i], t[i], acc);
         t[jj] = (jj == l) ? tau_j : (jj > l ? -tau_j * acc : 0.0);
     }
-    double *out = tn + (wy_base(N, C::LG, k) + j) * 64;
+    __syncwarp();
     if (lane < 8) {
 #pragma unroll
-        for (int jj = 0; jj < 8; ++jj) out[jj * 8 + l] = -t[jj];
+        for (int jj = 0; jj < 8; ++jj) Sm[warp][jj * 8 + l] = -t[jj];      // Sm = -T, row-major [i][j]
+    }
+    __syncwarp();
+    // Y[w][j] = sum_i V[w][i] (-T)[i][j]: M = rows of a tile, N = j, K = i (two k-chunks)
+    const double tb0 = Sm[warp][r * 8 + gq], tb1 = Sm[warp][(r + 4) * 8 + gq];
+    double *out = yb + (wy_base(N, C::LG, k) + j) * C::YBLK;
+#pragma unroll
+    for (int tt = 0; tt < C::NT; ++tt) {
+        double y0 = 0.0, y1 = 0.0;
+        dmma884(y0, y1, Vs[warp][r * SV + 8 * tt + gq], tb0, y0, y1);
+        dmma884(y0, y1, Vs[warp][(r + 4) * SV + 8 * tt + gq], tb1, y0, y1);
+        *reinterpret_cast<double2 *>(out + (8 * tt + gq) * 8 + 2 * r) = make_double2(y0, y1);
     }
 }
 
 // ---- staging one block (whole warp) -----------------------------------------------------------------
+// full barrier: 32 cp.async arrivals (one per lane) + 1 arrival carrying the bulk copy's byte count
 template <class C>
 __device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_t bar_full, int64_t k, int64_t b,
                                          int64_t id, int64_t FN1, int lane)
@@ -160,7 +179,13 @@ __device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_
     constexpr int NBW = C::NBW, W = C::W;
     const int i8 = lane & 7;
     const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
-    // VA[i][7 - i + r]: lanes run along r (256 contiguous bytes of hh_v per instruction)
+    // YB: the prepass wrote the shared-memory image; one bulk copy (TMA engine)
+    if (lane == 0) {
+        mbar_arrive_expect_tx(bar_full, C::YBLK * 8u);
+        bulk_g2s(smem_u32(stage + C::YB_OFF), a.tn + id * C::YBLK, C::YBLK * 8u, bar_full);
+    }
+    // VA[i][7 - i + r]: lanes run along r (256 contiguous bytes of hh_v per instruction); the skew
+    // 7 - i breaks the 16-byte alignment a bulk copy needs, hence 8-byte cp.async
 #pragma unroll
     for (int t = 0; t < 8 * NBW / 32; ++t) {
         const int i = (t * 32) / NBW;
@@ -168,15 +193,6 @@ __device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_
         const int64_t sl = __shfl_sync(0xffffffffu, slot, i);
         if (sl >= 0) cp_async8(smem_u32(stage + C::VA_OFF + i * W + 7 - i + rr), a.hh_v + sl * NBW + rr, 8u);
     }
-    // VB[7 - i + r][i]: lanes run along i (bank-conflict-light writes), 4 rows per instruction
-    if (slot >= 0) {
-#pragma unroll
-        for (int t = 0; t < NBW / 4; ++t) {
-            const int rr = t * 4 + (lane >> 3);
-            cp_async8(smem_u32(stage + C::VB_OFF + (7 - i8 + rr) * 8 + i8), a.hh_v + slot * NBW + rr, 8u);
-        }
-    }
-    cp_async16(smem_u32(stage + C::TN_OFF + 2 * lane), a.tn + id * 64 + 2 * lane, 16u);
     cp_async_mbar_arrive_noinc_wy(bar_full);
 }
 
@@ -320,8 +336,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             mbar_wait(bar_full + 8 * st, ph);
             const double *stage = ring + st * C::STAGE_DOUBLES;
             const double *va = stage + C::VA_OFF + gq * W + 2 * r;
-            const double *vb = stage + C::VB_OFF + gq * 8 + 2 * r;
-            const double *tn = stage + C::TN_OFF + gq * 8 + 2 * r;
+            const double *vb = stage + C::YB_OFF + gq * 8 + 2 * r;
 
             // --- D^T = x^T V: k-chunk (t, e) = rows 8t + 2r' + e; tile 0 (loaded last) goes last
             double D[NG][NACC][2];
@@ -341,23 +356,18 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
                     dmma884(D[g][NACC - 1][0], D[g][NACC - 1][1], t ? X[g][t][1] : T0[g][1], v2.y, D[g][NACC - 1][0],
                             D[g][NACC - 1][1]);
             }
-            // --- E^T = D^T (-T)^T
+            // --- E^T = D^T: T is folded into YB = V (-T), so the dot product feeds the update directly
             double E[NG][2];
-            {
-                const double2 t2 = *reinterpret_cast<const double2 *>(tn);
 #pragma unroll
-                for (int g = 0; g < NG; ++g) {
-                    double d0 = D[g][0][0], d1 = D[g][0][1];
-                    if (NACC == 2) {
-                        d0 += D[g][1][0];
-                        d1 += D[g][1][1];
-                    }
-                    double e0, e1;
-                    dmma884(e0, e1, d0, t2.x, 0.0, 0.0);
-                    dmma884(E[g][0], E[g][1], d1, t2.y, e0, e1);
+            for (int g = 0; g < NG; ++g) {
+                E[g][0] = D[g][0][0];
+                E[g][1] = D[g][0][1];
+                if (NACC == 2) {
+                    E[g][0] += D[g][1][0];
+                    E[g][1] += D[g][1][1];
                 }
             }
-            // --- x^T += E^T V^T, tile t -> registers of tile t+1 (the window moves up by 8 rows)
+            // --- x^T += E^T Y^T, tile t -> registers of tile t+1 (the window moves up by 8 rows)
 #pragma unroll
             for (int t = NT - 1; t >= 0; --t) {
                 const double2 v2 = *reinterpret_cast<const double2 *>(vb + 64 * t);
@@ -436,9 +446,10 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
     // the ring starts as zeros: the skew padding of VA / VB is never written by the copies, and
     // positions of reflectors outside a chain keep finite values (their row and column of T are 0)
     for (int i = threadIdx.x; i < C::OFF_BAR / 8; i += blockDim.x) ring[i] = 0.0;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
-            mbar_init(bar_full + 8 * i, 32);           // one cp.async arrival per lane of the staging warp
+            mbar_init(bar_full + 8 * i, 33);           // 32 cp.async arrivals + the bulk copy's expect_tx arrival
             mbar_init(bar_empty + 8 * i, (uint32_t)nact);
         }
         mbar_fence_init();
@@ -481,7 +492,7 @@ inline int wy_pick_P(int64_t nslab, int64_t K0, int nsm, int nw, int maxP)
 template <int NBW>
 size_t wy_tn_bytes(int64_t N)
 {
-    return (size_t)wy_nblocks(N, WyCfg<NBW>::LG) * 64 * sizeof(double);
+    return (size_t)wy_nblocks(N, WyCfg<NBW>::LG) * WyCfg<NBW>::YBLK * sizeof(double);
 }
 template <int NBW>
 size_t wy_scratch_bytes(int64_t N, int64_t nev)
@@ -512,8 +523,8 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
     }
-    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
-    wy_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)K0);
+    wy_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
