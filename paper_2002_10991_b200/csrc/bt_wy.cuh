@@ -268,6 +268,9 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq;
     const int64_t ldq8 = a.ldq << 3;
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
+    // warp-uniform fast path of the tile I/O: every column of the warp exists and 16-byte accesses
+    // are allowed; then only the first blocks of a chain (rows beyond N) need the guarded code
+    const bool fastio = a.align16 && (col0 + 8 * NG <= a.nev);
 
     // staging cursor: block it + NSP - LAG of this ring's sequence
     int64_t pk = grp, pb = bhi;
@@ -386,10 +389,29 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
                 if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
             }
             // --- tile NT-1 retires (rows 8b + nbw ..), the buffer of tile 0 is refilled
+            const int64_t bn = b - (PF2 ? 2 : 1);
+            if (fastio && (b << 3) + NBW + 8 <= N) {
+                double *pr = cb + (b << 3) + 2 * r;
 #pragma unroll
-            for (int g = 0; g < NG; ++g)
-                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
-            load_tile0(b - (PF2 ? 2 : 1), T0);
+                for (int g = 0; g < NG; ++g)
+                    *reinterpret_cast<double2 *>(pr + g * ldq8 + NBW) = make_double2(X[g][NT][0], X[g][NT][1]);
+                if (bn >= blo) {
+                    wait_prev(bn);
+                    const double *pl = cb + (bn << 3) + 2 * r;
+#pragma unroll
+                    for (int g = 0; g < NG; ++g) {
+                        const double2 v = CP ? __ldcg(reinterpret_cast<const double2 *>(pl + g * ldq8))
+                                             : *reinterpret_cast<const double2 *>(pl + g * ldq8);
+                        T0[g][0] = v.x;
+                        T0[g][1] = v.y;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int g = 0; g < NG; ++g)
+                    wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
+                load_tile0(bn, T0);
+            }
             ++it;
         };
 
