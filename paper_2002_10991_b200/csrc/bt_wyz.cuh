@@ -4,12 +4,12 @@
 //      H_7 .. H_0 = I - V T V^H,  T lower triangular, T[j][j] = tau_j,
 //      T[j][:j] = -tau_j (v_j^H V[:, :j]) T[:j, :j]                    (R2: tau as stored, v^H in the dot)
 //      D^T = x^T conj(V):  Dr = xr Vr + xi Vi,  Di = xi Vr - xr Vi      (four accumulators, 4 chains)
-//      E^T = D^T (-T)^T:   Er = Dr TNr - Di TNi, Ei = Dr TNi + Di TNr
-//      x^T += E^T V^T:     xr += Er Vr - Ei Vi,  xi += Er Vi + Ei Vr
+//      Y = V (-T)  (prepass, W x 8 complex):  the update operand, so no separate T product
+//      x^T += D^T Y^T:     xr += Dr Yr - Di Yi,  xi += Dr Yi + Di Yr
 // Registers hold x planar (real and imaginary fragments apart); global memory and shared memory
 // stay interleaved (re, im): one LDS.128 / LDG.128 = one complex element.  Interleaved 16-byte
 // elements keep the skewed rows of VA 16-byte aligned, so VA is staged with one bulk copy (TMA
-// engine) per reflector; VB (the transposed image) and -T by 16-byte cp.async.
+// engine) per reflector and YB with one more.
 #pragma once
 #include "bt_wy.cuh"
 
@@ -30,29 +30,33 @@ struct WyzCfg {
     // then differ by 4 banks (W*4 and 8*4 words are multiples of 32)
     static constexpr int SA = W + 1;                  // VA[i][w] row stride (elements)
     static constexpr int SB = 9;                      // VB[w][i] row stride (elements)
-    static constexpr int VA_OFF = 0;                  // offsets in doubles
-    static constexpr int VB_OFF = 2 * 8 * SA;
-    static constexpr int TN_OFF = VB_OFF + 2 * W * SB;
-    static constexpr int STAGE_DOUBLES = ((TN_OFF + 128 + 15) / 16) * 16;
+    static constexpr int VA_OFF = 0;                  // offsets in doubles; VA[i][w] = V
+    static constexpr int YB_OFF = 2 * 8 * SA;         // YB[w][j] = (V (-T))[w][j]
+    static constexpr int YBLK = 2 * W * SB;           // doubles of scratch per block (its YB image, padded rows)
+    static constexpr int STAGE_DOUBLES = ((YB_OFF + YBLK + 15) / 16) * 16;
+    static constexpr int PW = (NBW <= 64) ? 4 : 2;    // warps (= blocks) per CTA of the prepass kernel
     static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
-    static_assert((VB_OFF * 8) % 16 == 0 && (TN_OFF * 8) % 16 == 0, "16-byte aligned sections");
+    static_assert((YB_OFF * 8) % 16 == 0 && (YBLK * 8) % 16 == 0, "16-byte aligned sections");
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
-// ---- prepass: -T of every block (128 doubles: [n][k] interleaved) --------------------------------------
+// ---- prepass: Y = V (-T) of every block, as the padded YB[w][j] image (interleaved complex) --------------
 template <int NBW>
-__global__ void __launch_bounds__(256) wyz_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
-                                                          const double *__restrict__ hh_tau, double *__restrict__ tn)
+__global__ void __launch_bounds__(WyzCfg<NBW>::PW * 32) wyz_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
+                                                                           const double *__restrict__ hh_tau,
+                                                                           double *__restrict__ yb)
 {
     using C = WyzCfg<NBW>;
-    __shared__ double Sm[8][128];
+    constexpr int W = C::W, SV = W + 1;               // Vs row stride (elements)
+    __shared__ double Sm[C::PW][128];
+    __shared__ double Vs[C::PW][8 * SV * 2];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t k = blockIdx.y;
     const int64_t bhi = wy_bhi(N);
     const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
-    const int64_t j = (int64_t)blockIdx.x * 8 + warp;
+    const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
     if (j >= nblk) return;
     const int64_t b = bhi - j;
     const int64_t FN1 = hh_F(N - 1, C::LG);
@@ -65,7 +69,7 @@ __global__ void __launch_bounds__(256) wyz_prepass_kernel(int64_t N, const doubl
     // S = V^H V:  Sr = Vr^T Vr + Vi^T Vi,  Si = Vr^T Vi - Vi^T Vr
     double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0, p0 = 0.0, p1 = 0.0, q0 = 0.0, q1 = 0.0;
 #pragma unroll
-    for (int c = 0; c < C::W / 4; ++c) {
+    for (int c = 0; c < W / 4; ++c) {
         const int rl = 4 * c + r - (7 - gq);
         double vr = 0.0, vi = 0.0;
         if (slot >= 0 && rl >= 0 && rl < NBW) {
@@ -73,6 +77,7 @@ __global__ void __launch_bounds__(256) wyz_prepass_kernel(int64_t N, const doubl
             vr = v2.x;
             vi = v2.y;
         }
+        *reinterpret_cast<double2 *>(&Vs[warp][(gq * SV + 4 * c + r) * 2]) = make_double2(vr, vi);
         dmma884(a0, a1, vr, vr, a0, a1);
         dmma884(b0, b1, vi, vi, b0, b1);
         dmma884(p0, p1, vr, vi, p0, p1);
@@ -104,16 +109,47 @@ __global__ void __launch_bounds__(256) wyz_prepass_kernel(int64_t N, const doubl
         tr[jj] = (jj == l) ? tjr : (jj > l ? mr : 0.0);
         ti[jj] = (jj == l) ? tji : (jj > l ? mi : 0.0);
     }
-    double *out = tn + (wy_base(N, C::LG, k) + j) * 128;
+    __syncwarp();
     if (lane < 8) {
 #pragma unroll
-        for (int jj = 0; jj < 8; ++jj)
-            *reinterpret_cast<double2 *>(out + (jj * 8 + l) * 2) = make_double2(-tr[jj], -ti[jj]);
+        for (int jj = 0; jj < 8; ++jj) {                                   // Sm = -T, row-major [i][j]
+            Sm[warp][(jj * 8 + l) * 2] = -tr[jj];
+            Sm[warp][(jj * 8 + l) * 2 + 1] = -ti[jj];
+        }
     }
+    __syncwarp();
+    // Y[w][j] = sum_i V[w][i] T'[i][j], T' = -T:  Yr = Vr Tr' - Vi Ti',  Yi = Vr Ti' + Vi Tr'
+    double tbr[2], tbi[2];
+#pragma unroll
+    for (int c = 0; c < 2; ++c) {
+        tbr[c] = Sm[warp][((r + 4 * c) * 8 + gq) * 2];
+        tbi[c] = Sm[warp][((r + 4 * c) * 8 + gq) * 2 + 1];
+    }
+    double *out = yb + (wy_base(N, C::LG, k) + j) * C::YBLK;
+#pragma unroll
+    for (int tt = 0; tt < C::NT; ++tt) {
+        double yr0 = 0.0, yr1 = 0.0, yi0 = 0.0, yi1 = 0.0;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const double2 v2 = *reinterpret_cast<const double2 *>(&Vs[warp][((r + 4 * c) * SV + 8 * tt + gq) * 2]);
+            dmma884(yr0, yr1, v2.x, tbr[c], yr0, yr1);
+            dmma884(yr0, yr1, -v2.y, tbi[c], yr0, yr1);
+            dmma884(yi0, yi1, v2.x, tbi[c], yi0, yi1);
+            dmma884(yi0, yi1, v2.y, tbr[c], yi0, yi1);
+        }
+        double *o = out + ((8 * tt + gq) * C::SB + 2 * r) * 2;
+        *reinterpret_cast<double2 *>(o) = make_double2(yr0, yi0);
+        *reinterpret_cast<double2 *>(o + 2) = make_double2(yr1, yi1);
+    }
+    // the padding column (j = 8) of the image is never read; it is zeroed once so that the bulk copy moves
+    // defined bytes
+    for (int w = lane; w < W; w += 32) *reinterpret_cast<double2 *>(out + (w * C::SB + 8) * 2) = make_double2(0.0, 0.0);
 }
 
 // ---- staging one block (whole warp) ---------------------------------------------------------------------
-// full barrier: 32 cp.async arrivals (one per lane) + 1 arrival with the bulk-copy byte count
+// bulk copies (TMA engine) only: one per reflector for VA[i][7 - i + ..] (interleaved 16-byte elements keep
+// the skewed rows 16-byte aligned) and one for the YB image the prepass wrote.  Full barrier: one arrival
+// (lane 0) carrying the byte count.
 template <class C>
 __device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32_t bar_full, int64_t k, int64_t b,
                                           int64_t id, int64_t FN1, int lane)
@@ -121,24 +157,14 @@ __device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32
     constexpr int NBW = C::NBW;
     const int i8 = lane & 7;
     const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
-    // VA[i][7 - i + r]: one bulk copy per reflector (lanes 0..7), nbw * 16 bytes each
     const unsigned valid = __ballot_sync(0xffffffffu, slot >= 0) & 0xffu;
-    if (lane == 0) mbar_arrive_expect_tx(bar_full, (uint32_t)__popc(valid) * NBW * 16u);
+    if (lane == 0) {
+        mbar_arrive_expect_tx(bar_full, (uint32_t)__popc(valid) * NBW * 16u + C::YBLK * 8u);
+        bulk_g2s(smem_u32(stage + C::YB_OFF), a.tn + id * C::YBLK, C::YBLK * 8u, bar_full);
+    }
     __syncwarp();
     if (lane < 8 && slot >= 0)
         bulk_g2s(smem_u32(stage + C::VA_OFF + (i8 * C::SA + 7 - i8) * 2), a.hh_v + slot * NBW * 2, NBW * 16u, bar_full);
-    // VB[7 - i + r][i]: lanes run along i, 4 rows per instruction
-    if (slot >= 0) {
-#pragma unroll
-        for (int t = 0; t < NBW / 4; ++t) {
-            const int rr = t * 4 + (lane >> 3);
-            cp_async16(smem_u32(stage + C::VB_OFF + ((7 - i8 + rr) * C::SB + i8) * 2), a.hh_v + (slot * NBW + rr) * 2, 16u);
-        }
-    }
-    // -T: 64 elements
-    cp_async16(smem_u32(stage + C::TN_OFF + 2 * lane), a.tn + id * 128 + 2 * lane, 16u);
-    cp_async16(smem_u32(stage + C::TN_OFF + 64 + 2 * lane), a.tn + id * 128 + 64 + 2 * lane, 16u);
-    cp_async_mbar_arrive_noinc_wy(bar_full);
 }
 
 // ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column (interleaved in memory, planar in regs) ----
@@ -190,6 +216,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq * 2;
     const int64_t ldq8 = a.ldq << 4;
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
+    const bool fastio = col0 + 8 * NG <= a.nev;         // warp-uniform: every column of the warp exists
 
     int64_t pk = grp, pb = bhi;                         // staging cursor: block it + NSP - LAG of this ring
     auto advance = [&]() {
@@ -247,8 +274,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             mbar_wait(bar_full + 8 * st, ph);
             const double *stage = ring + st * C::STAGE_DOUBLES;
             const double *va = stage + C::VA_OFF + (gq * C::SA + 2 * r) * 2;   // + (8t + e) * 2
-            const double *vb = stage + C::VB_OFF + (gq * C::SB + 2 * r) * 2;   // + 8t * SB * 2 + e * 2
-            const double *tn = stage + C::TN_OFF + (gq * 8 + 2 * r) * 2;       // + e * 2
+            const double *vb = stage + C::YB_OFF + (gq * C::SB + 2 * r) * 2;   // + 8t * SB * 2 + e * 2
 
             // --- D^T = x^T conj(V): A1 = xr Vr, A2 = xi Vi, A3 = xi Vr, A4 = xr Vi
             double A1[NG][2], A2[NG][2], A3[NG][2], A4[NG][2];
@@ -271,33 +297,17 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                     }
                 }
             }
-            // --- E^T = D^T (-T)^T: Er = Dr TNr - Di TNi, Ei = Dr TNi + Di TNr
+            // --- E^T = D^T (T is folded into YB = V (-T)): Er = A1 + A2, Ei = A3 - A4
             double Er[NG][2], Ei[NG][2], nEi[NG][2];
-            {
-                const double2 t0 = *reinterpret_cast<const double2 *>(tn);
-                const double2 t1 = *reinterpret_cast<const double2 *>(tn + 2);
 #pragma unroll
-                for (int g = 0; g < NG; ++g) {
-                    const double dr0 = A1[g][0] + A2[g][0], dr1 = A1[g][1] + A2[g][1];
-                    const double di0 = A3[g][0] - A4[g][0], di1 = A3[g][1] - A4[g][1];
-                    double er0 = 0.0, er1 = 0.0, ei0 = 0.0, ei1 = 0.0;
-                    dmma884(er0, er1, dr0, t0.x, er0, er1);
-                    dmma884(ei0, ei1, dr0, t0.y, ei0, ei1);
-                    dmma884(er0, er1, -di0, t0.y, er0, er1);
-                    dmma884(ei0, ei1, di0, t0.x, ei0, ei1);
-                    dmma884(er0, er1, dr1, t1.x, er0, er1);
-                    dmma884(ei0, ei1, dr1, t1.y, ei0, ei1);
-                    dmma884(er0, er1, -di1, t1.y, er0, er1);
-                    dmma884(ei0, ei1, di1, t1.x, ei0, ei1);
-                    Er[g][0] = er0;
-                    Er[g][1] = er1;
-                    Ei[g][0] = ei0;
-                    Ei[g][1] = ei1;
-                    nEi[g][0] = -ei0;
-                    nEi[g][1] = -ei1;
+            for (int g = 0; g < NG; ++g)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    Er[g][e] = A1[g][e] + A2[g][e];
+                    Ei[g][e] = A3[g][e] - A4[g][e];
+                    nEi[g][e] = A4[g][e] - A3[g][e];
                 }
-            }
-            // --- x^T += E^T V^T: xr += Er Vr - Ei Vi, xi += Er Vi + Ei Vr; tile t -> registers of t+1
+            // --- x^T += E^T Y^T: xr += Er Yr - Ei Yi, xi += Er Yi + Ei Yr; tile t -> registers of t+1
 #pragma unroll
             for (int t = NT - 1; t >= 0; --t) {
                 const double2 v0 = *reinterpret_cast<const double2 *>(vb + 8 * t * C::SB * 2);
@@ -320,11 +330,36 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                 mbar_arrive(bar_empty + 8 * st);
                 if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
             }
+            if (fastio && (b << 3) + NBW + 8 <= N) {
+                // the block lies inside the matrix: no per-access guards (bt_wy.cuh)
+                double *pr = cb + 2 * ((b << 3) + 2 * r);
 #pragma unroll
-            for (int g = 0; g < NG; ++g)
-                wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
-                           Xi[g][NT][0], Xi[g][NT][1]);
-            load_tile0(b - 2, T0);
+                for (int g = 0; g < NG; ++g) {
+                    *reinterpret_cast<double2 *>(pr + g * ldq8 + 2 * NBW) = make_double2(Xr[g][NT][0], Xi[g][NT][0]);
+                    *reinterpret_cast<double2 *>(pr + g * ldq8 + 2 * NBW + 2) = make_double2(Xr[g][NT][1], Xi[g][NT][1]);
+                }
+                if (b - 2 >= blo) {
+                    wait_prev(b - 2);
+                    const double *pl = pr - 32;
+#pragma unroll
+                    for (int g = 0; g < NG; ++g) {
+                        const double2 v = CP ? __ldcg(reinterpret_cast<const double2 *>(pl + g * ldq8))
+                                             : *reinterpret_cast<const double2 *>(pl + g * ldq8);
+                        const double2 w = CP ? __ldcg(reinterpret_cast<const double2 *>(pl + g * ldq8 + 2))
+                                             : *reinterpret_cast<const double2 *>(pl + g * ldq8 + 2);
+                        T0[g][0] = v.x;
+                        T0[g][2] = v.y;
+                        T0[g][1] = w.x;
+                        T0[g][3] = w.y;
+                    }
+                }
+            } else {
+#pragma unroll
+                for (int g = 0; g < NG; ++g)
+                    wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
+                               Xi[g][NT][0], Xi[g][NT][1]);
+                load_tile0(b - 2, T0);
+            }
             ++it;
         };
 
@@ -375,7 +410,7 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     if (threadIdx.x == 0) {
         for (int i = 0; i < NS; ++i) {
-            mbar_init(bar_full + 8 * i, 33);           // 32 cp.async arrivals + the expect_tx arrival
+            mbar_init(bar_full + 8 * i, 1);            // lane 0 of the staging warp, with the byte count
             mbar_init(bar_empty + 8 * i, (uint32_t)nact);
         }
         mbar_fence_init();
@@ -402,7 +437,7 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
 template <int NBW>
 size_t wyz_tn_bytes(int64_t N)
 {
-    return (size_t)wy_nblocks(N, WyzCfg<NBW>::LG) * 128 * sizeof(double);
+    return (size_t)wy_nblocks(N, WyzCfg<NBW>::LG) * WyzCfg<NBW>::YBLK * sizeof(double);
 }
 template <int NBW>
 size_t wyz_scratch_bytes(int64_t N, int64_t nev)
@@ -433,8 +468,8 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
     }
-    const dim3 pgrid((unsigned)((wy_bhi(N) + 1 + 7) / 8), (unsigned)K0);
-    wyz_prepass_kernel<NBW><<<pgrid, 256, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)K0);
+    wyz_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
