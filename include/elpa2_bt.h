@@ -28,9 +28,10 @@
  * valid on the current CUDA device; hh_* are read-only.  The call enqueues work on `stream`
  * (a cudaStream_t passed as void*; NULL = the legacy default stream), returns without
  * synchronising the host (keep data on the device, no implicit synchronisation).
- * The default variant takes its scratch (64 / 128 doubles per block of 8 reflectors, about
- * N^2/(16 nbw) blocks) from a stream-ordered CUDA memory pool private to the library, which keeps
- * what it has allocated: in steady state a call allocates nothing new.  There is no CPU fallback: without a CUDA device every compute call
+ * The default variant takes its scratch (one (nbw+8) x 8 matrix per block of 8 reflectors, about
+ * N^2/(16 nbw) blocks: 0.55 N^2 doubles real, 1.2 N^2 doubles complex, i.e. 4.8 GB for N = 32768
+ * real) from a stream-ordered CUDA memory pool private to the library, which keeps what it has
+ * allocated: in steady state a call allocates nothing new.  There is no CPU fallback: without a CUDA device every compute call
  * fails with the cudaError_t of the launch.
  *
  * Return value: 0 on success; -i if the i-th argument (1-based: N=1, nbw=2, nev=3, hh_v=4,

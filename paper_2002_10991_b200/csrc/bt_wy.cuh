@@ -6,14 +6,14 @@
 //      H_7 .. H_1 H_0 = I - V T V^T,   T lower triangular, T[j][j] = tau_j,
 //      T[j][:j] = -tau_j (v_j^T V[:, :j]) T[:j, :j],
 // where V is the W x 8 matrix (W = nbw + 8 window rows 8b .. 8b+W-1) whose column i holds v_i at
-// row offset 7 - i.  Per block and per slab of 8 columns the window x (W x 8) is updated by
+// row offset 7 - i.  With Y = V (-T) (W x 8, computed once per block by wy_prepass_kernel) the
+// window x (W x 8 per slab of 8 columns) is updated by
 //      D^T = x^T V        (8 cols x 8 refl, K = W rows)       W/4  DMMAs
-//      E^T = D^T (-T)^T   (8 cols x 8 refl, K = 8)            2    DMMAs
-//      x^T += E^T V^T     (8 cols x W rows, K = 8)            W/4  DMMAs
-// i.e. (nbw/2 + 6) DMMAs for the nbw/2 DMMA-equivalents of useful work (4 L flops per reflector
-// and column): 84 % at nbw = 64.  All three products keep "column of q" on the M index of the
-// fragment (lane / 4) and permute the K index so that the C fragment of one product IS the A
-// fragment of the next: no shuffles, no shared-memory round trip for x, D or E.
+//      x^T += D^T Y^T     (8 cols x W rows, K = 8)            W/4  DMMAs
+// i.e. (nbw/2 + 4) DMMAs for the nbw/2 DMMA-equivalents of useful work (4 L flops per reflector
+// and column): 89 % at nbw = 64.  Both products keep "column of q" on the M index of the fragment
+// (lane / 4) and permute the K index so that the C fragment of the first product IS the A fragment
+// of the second: no shuffles, no shared-memory round trip for x or D.
 //
 //  * x^T fragment: lane (gq = lane/4, r = lane%4) holds rows 8t + 2r + {0,1} of column gq for
 //    every 8-row tile t of the window: NT = W/8 register pairs per slab.  This is the C layout of
@@ -21,13 +21,15 @@
 //    8t + 2r + e", the A layout of the dot product.
 //  * The window moves up by 8 rows = one tile per block: the update of tile t writes its result
 //    into the registers of tile t+1 (D != C in the DMMA), tile NT-1 retires to global memory
-//    (16 bytes per lane, 64 contiguous bytes per column), tile 0 is loaded for the next block.
-//  * V is staged in shared memory twice per block -- VA[i][w] (B fragments of the dot product) and
-//    VB[w][i] (B fragments of the update) -- by 8-byte cp.async straight from hh_v (the skew 7 - i
-//    breaks the 16-byte alignment bulk copies need); -T comes from a scratch array filled by
-//    wy_prepass_kernel (one warp per block: Gram matrix V^T V by DMMA, then the recurrence).
+//    (16 bytes per lane, 64 contiguous bytes per column), tile 0 is loaded one or two blocks ahead.
+//  * Shared memory per block: VA[i][w] = V (B fragments of the dot product), staged by 8-byte
+//    cp.async straight from hh_v (the skew 7 - i breaks the 16-byte alignment bulk copies need), and
+//    YB[w][j] = Y (B fragments of the update), one bulk copy (TMA engine) of the image the prepass
+//    left in the scratch array.
 //  * 8 warps per CTA (2 per SM sub-partition, 255 registers), no producer warp: the warps take
-//    turns at staging block it+NS-LAG; completion is tracked by cp.async.mbarrier.arrive.
+//    turns at staging block it+NS-LAG; completion is tracked on the stage's full mbarrier by
+//    cp.async.mbarrier.arrive and the bulk copy's byte count.
+//  * Few columns: chain-parallel mode (P warps per slab on interleaved chains, see prog_publish).
 //  * Order across chains: chain-major (R5), as in the other kernels.
 #pragma once
 #include "bt_common.cuh"
