@@ -219,7 +219,7 @@ def main() -> None:
     import numpy as np
     import torch
 
-    from paper_2002_10991_b200 import binding, synth_inputs as si
+    from paper_2002_10991_b200 import binding, shard, synth_inputs as si
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU path")
@@ -275,13 +275,9 @@ def main() -> None:
         barrier()
     clk = clocks.summary()
     step_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
-    total_ms = ev[0].elapsed_time(ev[args.steps])
-    t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms = float(t.item())
+    total_ms = shard.max_over_ranks(ev[0].elapsed_time(ev[args.steps]), dist, "cuda")
     ms_per_step = total_ms / args.steps
-    value = world * flops / (ms_per_step * 1e-3) / 1e9
+    value = shard.aggregate_throughput(flops, world, ms_per_step * 1e-3) / 1e9
 
     # unitarity check on the timed buffer (every H is unitary, so column norms must not move)
     nrm = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
@@ -302,11 +298,7 @@ def main() -> None:
             binding.trans_ev_tridi_to_band_host(N, nbw, hv_np, ht_np, q_np)
             launches += binding.last_launch_count()
         torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dt = float(t.item())
+        dt = shard.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
         h2d = (G * nbw + G + N * nev) * esz
         d2h = N * nev * esz
         e2e = {"value": world * flops * args.e2e_steps / dt / 1e9, "unit": "GFLOP/s",
