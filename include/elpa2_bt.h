@@ -69,6 +69,20 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
                                       const void *hh_v, const void *hh_tau,
                                       void *q, int64_t ldq);
 
+/* SURVEY.md 8(f) NEXT-1, first version (real FP64 only): bulge chasing of a symmetric band matrix to
+ * tridiagonal form on the device (Eq. 6b; the step is SURVEY.md 8(c) O3 / DESIGN.md
+ * R3, R4, R7), emitting the reflectors in the layout the calls above consume.
+ *   ab:  DEVICE, (2*nbw+1) x N doubles, column j at ab + j*(2*nbw+1), ab[(i-j) + j*(2*nbw+1)] = B[i][j]
+ *        for 0 <= i-j <= nbw (lower band; rows nbw+1 .. 2*nbw of every column are room for the
+ *        fill and must be zero on entry).  Overwritten with the tridiagonal matrix T.
+ *   hh_v (G*nbw), hh_tau (G): DEVICE outputs, every slot written (identity slots: v = e1, tau = 0).
+ *   d (N), e (N-1): DEVICE outputs, diagonal and sub-diagonal of T = Q2^T B Q2.
+ * Asynchronous on `stream`: about 3N kernel launches (one per wavefront 3s + k of independent
+ * chase steps), no host synchronisation, no allocation.  Returns 0; -i for a bad i-th argument
+ * (N=1, nbw=2, ab=3, hh_v=4, hh_tau=5, d=6, e=7); > 0 = cudaError_t.  N = 0: no work. */
+int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh_tau,
+                        double *d, double *e, void *stream);
+
 /* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */
 int64_t elpa2_hh_count(int64_t N, int nbw);
 /* first slot of sweep s (s in [0, N-1]; s = N-1 gives G); -1 if out of range */

@@ -1,0 +1,168 @@
+// bc_chase.cuh -- SURVEY.md 8(f) NEXT-1, first version: bulge chasing of a real symmetric band matrix
+// to tridiagonal form on the GPU (Eq. 6b), emitting the Householder reflectors
+// directly in the device layout the back-transformation consumes (include/elpa2_bt.h).
+//
+// Step (s, k) -- sweep s, chase block k -- is exactly the oracle's step (R3, R7):
+//   rows r0 = s+1+k nbw .. r1 = min(s+(k+1) nbw, N-1), eliminated column c = s (k = 0) or r0-nbw;
+//   (v, tau, beta) from B[r0..r1][c]; B <- H^T B H on the three blocks that can be non-zero:
+//   (i) B[r0..r1][c+1..r0-1], (ii) the diagonal block (symmetric rank-2 form), (iii) the block below.
+// Parallelism: step (s+1, k) touches what steps (s+1, k-1) and (s, k+2) wrote (the latter's head
+// element is the corner of the former's block (iii)), and steps with equal 3s + k touch disjoint
+// rectangles of the lower band.  So wavefront t = 3s + k runs as ONE launch with one CTA per step
+// (about N / (3 nbw) CTAs), and stream order provides the dependency between wavefronts.
+// The band lives in global memory (L2-resident: (2 nbw + 1) N doubles); a CTA keeps v and the
+// two work vectors of block (ii) in shared memory.  Every sum runs in the order SURVEY O3 / the oracle
+// states and every product and sum is rounded separately (__dmul_rn / __dadd_rn: no FMA contraction):
+// the tridiagonal form is unique but ill-conditioned (it is the Lanczos recurrence started at e1), so
+// two backward-stable chases drift apart entry by entry as N grows; rounding exactly like the
+// definition keeps the result reproducible and element-wise comparable at any N.
+#pragma once
+#include "bt_common.cuh"
+
+namespace elpa2bt {
+
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t, int64_t s_hi, double *__restrict__ ab,
+                                                           double *__restrict__ hh_v, double *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    constexpr int64_t ldab = 2 * NBW + 1;
+    __shared__ double v[NBW], p[NBW], w2[NBW], red[128];
+    __shared__ double s_tau, s_scal, s_beta;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    const int64_t r0 = s + 1 + (k << LG);
+    int64_t r1 = s + ((k + 1) << LG);
+    if (r1 > N - 1) r1 = N - 1;
+    const int L = (int)(r1 - r0 + 1);
+    const int64_t c = (k == 0) ? s : r0 - NBW;
+    const int64_t g = hh_off(N, LG, s) + k;
+#define BC_B(i, j) ab[((i) - (j)) + (j) * ldab]
+    double *vout = hh_v + g * NBW;
+    if (k > 0 && L == 1) {                       // nothing to eliminate: identity slot (R3)
+        for (int i = tid; i < NBW; i += nt) vout[i] = (i == 0) ? 1.0 : 0.0;
+        if (tid == 0) hh_tau[g] = 0.0;
+        return;
+    }
+    // --- Householder generator (R7): beta = -sign(alpha) ||x||, tau = (beta - alpha)/beta, v = x/(alpha - beta)
+    if (tid < L) p[tid] = BC_B(r0 + tid, c);     // x, parked in p
+    __syncthreads();
+    if (tid == 0) {
+        const double alpha = p[0];
+        double ss = 0.0;
+        for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
+        if (ss == 0.0) {
+            s_tau = 0.0;
+            s_scal = 0.0;
+            s_beta = alpha;
+        } else {
+            const double nrm = sqrt(__dadd_rn(__dmul_rn(alpha, alpha), ss));
+            const double b = (alpha >= 0.0) ? -nrm : nrm;
+            s_tau = __ddiv_rn(__dsub_rn(b, alpha), b);
+            s_scal = __ddiv_rn(1.0, __dsub_rn(alpha, b));
+            s_beta = b;
+        }
+    }
+    __syncthreads();
+    const double tau = s_tau;
+    for (int i = tid; i < NBW; i += nt) {
+        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], s_scal) : 0.0);
+        v[i] = vi;
+        vout[i] = vi;
+    }
+    __syncthreads();
+    if (tid < L) BC_B(r0 + tid, c) = (tid == 0) ? s_beta : 0.0;
+    if (tid == 0) hh_tau[g] = tau;
+    if (tau == 0.0) return;
+    // --- (i) A <- H^T A on the rest of the bulge block: one thread per column
+    for (int64_t j = c + 1 + tid; j < r0; j += nt) {
+        double dot = 0.0;
+        for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BC_B(r0 + i, j)));
+        for (int i = 0; i < L; ++i) BC_B(r0 + i, j) = __dsub_rn(BC_B(r0 + i, j), __dmul_rn(__dmul_rn(tau, v[i]), dot));
+    }
+    // --- (ii) D <- H^T D H: p = D v;  M = D - tau v p^T;  w2 = M v;  D' = M - tau w2 v^T (lower part)
+    __syncthreads();                              // p held x until here
+    for (int j = tid; j < L; j += nt) {
+        double dot = 0.0;
+        for (int i = 0; i < L; ++i)
+            dot = __dadd_rn(dot, __dmul_rn(v[i], (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i)));
+        red[j] = dot;
+    }
+    __syncthreads();
+    for (int i = tid; i < L; i += nt) {
+        double dot = 0.0;
+        for (int j = 0; j < L; ++j) {
+            const double dij = (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i);
+            const double m = __dsub_rn(dij, __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+            dot = __dadd_rn(dot, __dmul_rn(m, v[j]));
+        }
+        w2[i] = dot;
+    }
+    __syncthreads();
+    for (int j = tid; j < L; j += nt)
+        for (int i = j; i < L; ++i) {
+            const double m = __dsub_rn(BC_B(r0 + i, r0 + j), __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+            BC_B(r0 + i, r0 + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
+        }
+    // --- (iii) E <- E H on the block below: one thread per row; creates the next bulge
+    int64_t r2 = r1 + NBW;
+    if (r2 > N - 1) r2 = N - 1;
+    for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
+        double dot = 0.0;
+        for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BC_B(i, r0 + l), v[l]));
+        for (int l = 0; l < L; ++l) BC_B(i, r0 + l) = __dsub_rn(BC_B(i, r0 + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
+    }
+#undef BC_B
+}
+
+// d[i] = T[i][i], e[i] = T[i+1][i]
+template <int NBW>
+__global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, double *__restrict__ d, double *__restrict__ e)
+{
+    constexpr int64_t ldab = 2 * NBW + 1;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) d[i] = ab[i * ldab];
+    if (i + 1 < N) e[i] = ab[1 + i * ldab];
+}
+
+// host: all wavefronts t = 3s + k, in order, on one stream.  *launches = kernels launched.
+template <int NBW>
+cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_tau, double *d, double *e,
+                               cudaStream_t st, int64_t *launches)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    int64_t nl = 0;
+    if (N >= 2) {
+        const int64_t Kmax = (N - 2 + NBW) >> LG;                  // K(0)
+        // last wavefront: max over s of 3s + K(s) - 1; K(s) >= 1 for s <= N-2, so s = N-2 gives 3(N-2)
+        int64_t tmax = 0;
+        for (int64_t s = (N > 2 + Kmax) ? N - 2 - Kmax : 0; s <= N - 2; ++s) {
+            const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+            if (3 * s + K - 1 > tmax) tmax = 3 * s + K - 1;
+        }
+        if (Kmax - 1 > tmax) tmax = Kmax - 1;
+        for (int64_t t = 0; t <= tmax; ++t) {
+            int64_t s_hi = t / 3;
+            if (s_hi > N - 2) s_hi = N - 2;
+            int64_t s_lo = (t - Kmax + 1 + 2) / 3;                 // k = t - 3s <= Kmax - 1
+            if (t - Kmax + 1 <= 0) s_lo = 0;
+            if (s_lo > s_hi) continue;
+            bc_wavefront_kernel<NBW><<<(unsigned)(s_hi - s_lo + 1), 128, 0, st>>>(N, t, s_hi, ab, hh_v, hh_tau);
+            ++nl;
+        }
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return e1;
+    }
+    if (N >= 1) {
+        bc_extract_kernel<NBW><<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ab, d, e);
+        ++nl;
+    }
+    if (launches) *launches = nl;
+    return cudaGetLastError();
+}
+
+}  // namespace elpa2bt

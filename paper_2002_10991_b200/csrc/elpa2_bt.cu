@@ -13,6 +13,7 @@
 #include "bt_simple.cuh"
 #include "bt_wy.cuh"
 #include "bt_wyz.cuh"
+#include "bc_chase.cuh"
 
 using namespace elpa2bt;
 
@@ -246,6 +247,31 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
     if (rc != 0) return rc;
     if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
     if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
+    return 0;
+}
+
+int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh_tau, double *d, double *e,
+                        void *stream)
+{
+    if (N < 0) return -1;
+    if (lg_of(nbw) < 0) return -2;
+    g_last_launches = 0;
+    if (N == 0) return 0;
+    if (!ab) return -3;
+    if (N >= 2 && !hh_v) return -4;
+    if (N >= 2 && !hh_tau) return -5;
+    if (!d) return -6;
+    if (N >= 2 && !e) return -7;
+    cudaStream_t st = (cudaStream_t)stream;
+    int64_t nl = 0;
+    cudaError_t err;
+    switch (nbw) {
+    case 32: err = launch_bulge_chase<32>(N, ab, hh_v, hh_tau, d, e, st, &nl); break;
+    case 64: err = launch_bulge_chase<64>(N, ab, hh_v, hh_tau, d, e, st, &nl); break;
+    default: err = launch_bulge_chase<128>(N, ab, hh_v, hh_tau, d, e, st, &nl); break;
+    }
+    if (err != cudaSuccess) return (int)err;
+    g_last_launches = (int)(nl > 0x7fffffff ? 0x7fffffff : nl);
     return 0;
 }
 

@@ -99,6 +99,42 @@ def test_chain_parallel_mode(nbw, cplx):
 
 
 @pytest.mark.parametrize("cplx", [False, True])
+def test_more_columns_than_one_wave(cplx):
+    # more slabs than 148 CTAs x 8 warps x NGMAX: the grid becomes a multiple of the SM count > 1
+    nev = 148 * 8 * 8 * (2 if cplx else 4) + 8 * 31 + 3
+    _check(70, 32, nev, cplx)
+
+
+def test_repeated_and_concurrent_calls_share_the_scratch_pool():
+    """Two streams, interleaved calls on different problems: every call takes its scratch from the
+    stream-ordered pool, so neither host synchronisation nor cross-talk may occur."""
+    import torch
+
+    from paper_2002_10991_b200 import binding
+    from gpu_util import to_device_colmajor
+
+    probs = []
+    for (N, nbw, nev, seed) in ((300, 64, 64, 1), (17 * 32 + 1, 32, 9, 2), (260, 128, 40, 3)):
+        hh_v, hh_tau, _, _ = _reflectors(N, nbw, 90 + seed, False)
+        x = _x(N, nev, seed, False)
+        probs.append((N, nbw, torch.from_numpy(hh_v).cuda(), torch.from_numpy(hh_tau).cuda(), x,
+                      oracle_apply(N, nbw, hh_v, hh_tau, x)))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    outs = []
+    for rep in range(3):
+        for i, (N, nbw, dv, dt, x, want) in enumerate(probs):
+            s = streams[(i + rep) % 2]
+            with torch.cuda.stream(s):
+                q = to_device_colmajor(x)
+                binding.trans_ev_tridi_to_band(N, nbw, dv, dt, q, stream=s)
+            outs.append((q, want, x))
+    torch.cuda.synchronize()
+    for q, want, x in outs:
+        assert np.abs(q.cpu().numpy() - want).max() <= TOL * np.abs(x).max()
+
+
+@pytest.mark.parametrize("cplx", [False, True])
 def test_simple_variant_matches_oracle(cplx):
     _check(150, 32, 37, cplx, variant=1)
     _check(300, 64, 21, cplx, variant=1)
