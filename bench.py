@@ -51,7 +51,7 @@ METRIC = "back-transform FP64 GFLOP/s (2N^2*nev real / 8N^2*nev cplx)"
 # FP64 ALU roofline: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full), by config
-NCU_TRAFFIC_BYTES = {4: 2.305307e12 + 2.203028e12}    # profiles/r1_b_wy_config4.md
+NCU_TRAFFIC_BYTES = {4: 2.603878e12 + 2.202669e12}    # profiles/r1_c_wy_config4.md
 
 
 def model_flops(cplx: bool, N: int, nev: int) -> float:
