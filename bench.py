@@ -188,6 +188,65 @@ def run_reference(args, rank: int) -> None:
     }), flush=True)
 
 
+def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
+    """--chase: SURVEY.md 8(f) NEXT-1, first version.  One step = one band -> tridiagonal reduction of the
+    config's seeded band matrix on the device (about 3N wavefront launches); model work 6 N^2 nbw flops
+    (SURVEY O3).  Replicas only: the chase does not shard."""
+    import numpy as np
+    import torch
+
+    from paper_2002_10991_b200 import binding, shard, synth_inputs as si
+
+    if cplx:
+        raise SystemExit("--chase: real configs only in this version (1, 2, 4)")
+    ab_h = torch.from_numpy(np.ascontiguousarray(si.band_matrix(N, nbw, seed, False).T)).pin_memory()
+    ab = torch.empty_like(ab_h, device="cuda")
+    flops = 6.0 * float(N) * float(N) * nbw
+    stream = torch.cuda.current_stream()
+    times, launches = [], 0
+    dfma_tf = binding.probe_fp64(0, 8192, 20)
+    with ClockSampler(local_rank) as clocks:
+        for i in range(args.warmup + args.steps):
+            ab.copy_(ab_h, non_blocking=True)          # the chase overwrites its input: restore, untimed
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(stream)
+            hv, ht, d, e = binding.bulge_chase(N, nbw, ab, stream=stream)
+            e1.record(stream)
+            torch.cuda.synchronize()
+            if i >= args.warmup:
+                times.append(e0.elapsed_time(e1))
+                launches += binding.last_launch_count()
+    ms = shard.max_over_ranks(sum(times) / len(times), None)
+    # sanity of the result that was timed: T has the eigenvalue sum (trace) of B
+    tr_err = abs(float(d.sum().item()) - float(ab_h[:, 0].sum().item())) / max(1.0, float(ab_h[:, 0].abs().sum().item()))
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+
+        Ns = min(N, 4096)                               # bounded sample: work grows like N^2
+        ab_s = si.band_matrix(Ns, nbw, seed, False)
+        t0 = time.perf_counter()
+        oracle.bulge_chase(ab_s, nbw)
+        ts = time.perf_counter() - t0
+        cpu = {"value": 6.0 * Ns * Ns * nbw / ts / 1e9, "unit": "GFLOP/s", "cores": 1, "kind": "oracle", "seconds": ts,
+               "sample": f"the same seeded band matrix truncated to N = {Ns} (single thread: the chase is sequential)"}
+    if rank == 0:
+        achieved = flops / (ms * 1e-3) / 1e12
+        print(json.dumps({
+            "metric": "bulge chase FP64 GFLOP/s (6 N^2 nbw)", "value": world * flops / (ms * 1e-3) / 1e9, "unit": "GFLOP/s",
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"bulge chase of config {args.config}'s band matrix: real FP64 N={N} nbw={nbw}",
+                       "parallelism": "replicas only", "l2": "band matrix restored from host before every step"},
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": dfma_tf, "unit": "TFLOP/s", "frac": achieved / dfma_tf,
+                         "peak_source": "DFMA probe of this run; first version: launch- and latency-bound",
+                         "kernel": "bc_wavefront_kernel", "kernel_ms": ms, "traffic": None},
+            "clocks": clocks.summary(), "e2e": None, "gpu_launches": launches, "cpu_baseline": cpu,
+            "checks": {"relative_trace_error": tr_err},
+        }), flush=True)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -197,6 +256,8 @@ def main() -> None:
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer calls (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--chase", action="store_true",
+                    help="time SURVEY 8(f) NEXT-1 instead: the GPU bulge chase (real configs) that produces the reflectors")
     ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",
                     help="profiling aid: replace the chosen config's shape (named 'custom' in the output)")
     args = ap.parse_args()
@@ -233,6 +294,9 @@ def main() -> None:
     cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
     esz = 16 if cplx else 8
     flops = model_flops(cplx, N, nev)
+    if args.chase:
+        run_chase(args, N, nbw, cplx, seed_r, rank, world, local_rank)
+        return
 
     # ---- inputs, generated on the device (each rank: its own nev columns, same reflectors) ----
     lengths = binding.hh_lengths(N, nbw)

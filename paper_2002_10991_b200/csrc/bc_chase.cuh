@@ -119,6 +119,162 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
 #undef BC_B
 }
 
+// ---- the same step with its three blocks staged in shared memory (nbw <= 64) -------------------------
+// In band storage every column j of the step's region is ONE contiguous segment: rows r0..r1 for
+// c < j < r0 (block i), rows j..r2 for r0 <= j <= r1 (lower part of block ii + block iii).  The CTA
+// copies those segments into a tile S[col][row - r0] (column stride odd: conflict-free both ways),
+// runs the step there with exactly the arithmetic of bc_wavefront_kernel, and copies them back.
+template <int NBW>
+__global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64_t t, int64_t s_hi,
+                                                                double *__restrict__ ab, double *__restrict__ hh_v,
+                                                                double *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : 6;
+    constexpr int64_t ldab = 2 * NBW + 1;
+    constexpr int LDS = 2 * NBW + 1;              // tile column stride (doubles)
+    extern __shared__ double S[];                 // (2 NBW - 1) columns x LDS
+    __shared__ double v[NBW], p[NBW], w2[NBW];
+    __shared__ double s_tau, s_scal, s_beta;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    const int64_t r0 = s + 1 + (k << LG);
+    int64_t r1 = s + ((k + 1) << LG);
+    if (r1 > N - 1) r1 = N - 1;
+    const int L = (int)(r1 - r0 + 1);
+    const int64_t c = (k == 0) ? s : r0 - NBW;
+    const int64_t g = hh_off(N, LG, s) + k;
+    double *vout = hh_v + g * NBW;
+    if (k > 0 && L == 1) {
+        for (int i = tid; i < NBW; i += nt) vout[i] = (i == 0) ? 1.0 : 0.0;
+        if (tid == 0) hh_tau[g] = 0.0;
+        return;
+    }
+    int64_t r2 = r1 + NBW;
+    if (r2 > N - 1) r2 = N - 1;
+    const int nA = (int)(r0 - c - 1);             // columns of block (i): c+1 .. r0-1
+    const int nR = (int)(r2 - r0 + 1);            // tile rows: r0 .. r2
+    const int ncol = nA + L;                      // tile columns: c+1 .. r1
+    // tile column q <-> matrix column c+1+q; element (row, col) at S[q * LDS + row - r0]
+    auto seg = [&](int q, int &lo, int &hi) {     // local rows [lo, hi) stored for tile column q
+        if (q < nA) {
+            lo = 0;
+            hi = L;
+        } else {
+            lo = q - nA;
+            hi = nR;
+        }
+    };
+    // --- stage in: flat loop over (column, row) so that many independent loads are in flight; lanes run
+    //     along the contiguous band segment of a column
+    const int nRp = (nR + 31) & ~31;
+#pragma unroll 4
+    for (int e = tid; e < ncol * nRp; e += nt) {
+        const int q = e / nRp, row = e - q * nRp;
+        int lo, hi;
+        seg(q, lo, hi);
+        if (row >= lo && row < hi) {
+            const int64_t j = c + 1 + q;
+            S[q * LDS + row] = ab[(r0 + row - j) + j * ldab];
+        }
+    }
+    if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];       // x = B[r0..r1][c]
+    __syncthreads();
+#define BS(rl, q) S[(q) * LDS + (rl)]
+    if (tid == 0) {
+        const double alpha = p[0];
+        double ss = 0.0;
+        for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
+        if (ss == 0.0) {
+            s_tau = 0.0;
+            s_scal = 0.0;
+            s_beta = alpha;
+        } else {
+            const double nrm = sqrt(__dadd_rn(__dmul_rn(alpha, alpha), ss));
+            const double b = (alpha >= 0.0) ? -nrm : nrm;
+            s_tau = __ddiv_rn(__dsub_rn(b, alpha), b);
+            s_scal = __ddiv_rn(1.0, __dsub_rn(alpha, b));
+            s_beta = b;
+        }
+    }
+    __syncthreads();
+    const double tau = s_tau;
+    for (int i = tid; i < NBW; i += nt) {
+        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], s_scal) : 0.0);
+        v[i] = vi;
+        vout[i] = vi;
+    }
+    if (tid < L) ab[(r0 + tid - c) + c * ldab] = (tid == 0) ? s_beta : 0.0;
+    if (tid == 0) hh_tau[g] = tau;
+    __syncthreads();
+    if (tau == 0.0) return;                       // the tile is unchanged: nothing to copy back
+    // Blocks (i), (ii), (iii) are disjoint and only read v: three groups of 64 threads run them side by
+    // side; the two internal barriers of (ii) are named barriers of its own 64 threads.
+    const int grp = tid >> 6, t64 = tid & 63;
+    if (grp == 0) {
+        // --- (i): one thread per column q < nA
+        for (int q = t64; q < nA; q += 64) {
+            double dot = 0.0;
+#pragma unroll 8
+            for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BS(i, q)));
+#pragma unroll 8
+            for (int i = 0; i < L; ++i) BS(i, q) = __dsub_rn(BS(i, q), __dmul_rn(__dmul_rn(tau, v[i]), dot));
+        }
+    } else if (grp == 1) {
+        // --- (iii): one thread per row L .. nR-1
+        for (int rl = L + t64; rl < nR; rl += 64) {
+            double dot = 0.0;
+#pragma unroll 8
+            for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BS(rl, nA + l), v[l]));
+#pragma unroll 8
+            for (int l = 0; l < L; ++l)
+                BS(rl, nA + l) = __dsub_rn(BS(rl, nA + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
+        }
+    } else if (grp == 2) {
+        // --- (ii): D(i, j) = BS(max, nA + min);  p = D v;  M = D - tau v p^T;  w2 = M v;  D' = M - tau w2 v^T
+        for (int j = t64; j < L; j += 64) {
+            double dot = 0.0;
+#pragma unroll 8
+            for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], (i >= j) ? BS(i, nA + j) : BS(j, nA + i)));
+            p[j] = dot;
+        }
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        for (int i = t64; i < L; i += 64) {
+            double dot = 0.0;
+#pragma unroll 8
+            for (int j = 0; j < L; ++j) {
+                const double dij = (i >= j) ? BS(i, nA + j) : BS(j, nA + i);
+                const double m = __dsub_rn(dij, __dmul_rn(__dmul_rn(tau, v[i]), p[j]));
+                dot = __dadd_rn(dot, __dmul_rn(m, v[j]));
+            }
+            w2[i] = dot;
+        }
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        for (int j = t64; j < L; j += 64)
+#pragma unroll 4
+            for (int i = j; i < L; ++i) {
+                const double m = __dsub_rn(BS(i, nA + j), __dmul_rn(__dmul_rn(tau, v[i]), p[j]));
+                BS(i, nA + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
+            }
+    }
+    __syncthreads();
+#undef BS
+    // --- stage out
+#pragma unroll 4
+    for (int e = tid; e < ncol * nRp; e += nt) {
+        const int q = e / nRp, row = e - q * nRp;
+        int lo, hi;
+        seg(q, lo, hi);
+        if (row >= lo && row < hi) {
+            const int64_t j = c + 1 + q;
+            ab[(r0 + row - j) + j * ldab] = S[q * LDS + row];
+        }
+    }
+}
+
 // d[i] = T[i][i], e[i] = T[i+1][i]
 template <int NBW>
 __global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, double *__restrict__ d, double *__restrict__ e)
@@ -136,6 +292,16 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     int64_t nl = 0;
+    constexpr int smem_bytes = (2 * NBW - 1) * (2 * NBW + 1) * 8;
+    if (NBW <= 64) {
+        static bool attr_done = false;
+        if (!attr_done) {
+            cudaError_t e0 = cudaFuncSetAttribute(bc_wavefront_smem_kernel<(NBW <= 64 ? NBW : 64)>,
+                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+            if (e0 != cudaSuccess) return e0;
+            attr_done = true;
+        }
+    }
     if (N >= 2) {
         const int64_t Kmax = (N - 2 + NBW) >> LG;                  // K(0)
         // last wavefront: max over s of 3s + K(s) - 1; K(s) >= 1 for s <= N-2, so s = N-2 gives 3(N-2)
@@ -151,7 +317,11 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
             int64_t s_lo = (t - Kmax + 1 + 2) / 3;                 // k = t - 3s <= Kmax - 1
             if (t - Kmax + 1 <= 0) s_lo = 0;
             if (s_lo > s_hi) continue;
-            bc_wavefront_kernel<NBW><<<(unsigned)(s_hi - s_lo + 1), 128, 0, st>>>(N, t, s_hi, ab, hh_v, hh_tau);
+            if (NBW <= 64)
+                bc_wavefront_smem_kernel<(NBW <= 64 ? NBW : 64)>
+                    <<<(unsigned)(s_hi - s_lo + 1), 256, smem_bytes, st>>>(N, t, s_hi, ab, hh_v, hh_tau);
+            else
+                bc_wavefront_kernel<NBW><<<(unsigned)(s_hi - s_lo + 1), 128, 0, st>>>(N, t, s_hi, ab, hh_v, hh_tau);
             ++nl;
         }
         cudaError_t e1 = cudaGetLastError();
