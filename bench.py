@@ -197,11 +197,9 @@ def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
 
     from paper_2002_10991_b200 import binding, shard, synth_inputs as si
 
-    if cplx:
-        raise SystemExit("--chase: real configs only in this version (1, 2, 4)")
-    ab_h = torch.from_numpy(np.ascontiguousarray(si.band_matrix(N, nbw, seed, False).T)).pin_memory()
+    ab_h = torch.from_numpy(np.ascontiguousarray(si.band_matrix(N, nbw, seed, cplx).T)).pin_memory()
     ab = torch.empty_like(ab_h, device="cuda")
-    flops = 6.0 * float(N) * float(N) * nbw
+    flops = (24.0 if cplx else 6.0) * float(N) * float(N) * nbw
     stream = torch.cuda.current_stream()
     times, launches = [], 0
     dfma_tf = binding.probe_fp64(0, 8192, 20)
@@ -219,29 +217,32 @@ def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
                 launches += binding.last_launch_count()
     ms = shard.max_over_ranks(sum(times) / len(times), None)
     # sanity of the result that was timed: T has the eigenvalue sum (trace) of B
-    tr_err = abs(float(d.sum().item()) - float(ab_h[:, 0].sum().item())) / max(1.0, float(ab_h[:, 0].abs().sum().item()))
+    diag = ab_h[:, 0].real if cplx else ab_h[:, 0]
+    tr_err = abs(float(d.sum().item()) - float(diag.sum().item())) / max(1.0, float(diag.abs().sum().item()))
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         import oracle
 
-        Ns = min(N, 4096)                               # bounded sample: work grows like N^2
-        ab_s = si.band_matrix(Ns, nbw, seed, False)
+        Ns = min(N, 2048 if cplx else 4096)             # bounded sample: work grows like N^2
+        ab_s = si.band_matrix(Ns, nbw, seed, cplx)
         t0 = time.perf_counter()
         oracle.bulge_chase(ab_s, nbw)
         ts = time.perf_counter() - t0
-        cpu = {"value": 6.0 * Ns * Ns * nbw / ts / 1e9, "unit": "GFLOP/s", "cores": 1, "kind": "oracle", "seconds": ts,
+        cpu = {"value": (24.0 if cplx else 6.0) * Ns * Ns * nbw / ts / 1e9, "unit": "GFLOP/s", "cores": 1, "kind": "oracle", "seconds": ts,
                "sample": f"the same seeded band matrix truncated to N = {Ns} (single thread: the chase is sequential)"}
     if rank == 0:
         achieved = flops / (ms * 1e-3) / 1e12
         print(json.dumps({
-            "metric": "bulge chase FP64 GFLOP/s (6 N^2 nbw)", "value": world * flops / (ms * 1e-3) / 1e9, "unit": "GFLOP/s",
+            "metric": "bulge chase FP64 GFLOP/s (6 N^2 nbw real / 24 N^2 nbw cplx)", "value": world * flops / (ms * 1e-3) / 1e9, "unit": "GFLOP/s",
             "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"bulge chase of config {args.config}'s band matrix: real FP64 N={N} nbw={nbw}",
+            "config": {"workload": f"bulge chase of config {args.config}'s band matrix: "
+                                   f"{'complex' if cplx else 'real'} FP64 N={N} nbw={nbw}",
                        "parallelism": "replicas only", "l2": "band matrix restored from host before every step"},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": dfma_tf, "unit": "TFLOP/s", "frac": achieved / dfma_tf,
                          "peak_source": "DFMA probe of this run; first version: launch- and latency-bound",
-                         "kernel": "bc_wavefront_kernel", "kernel_ms": ms, "traffic": None},
+                         "kernel": "bc_wavefront_kernel_z" if cplx else "bc_wavefront_smem_kernel", "kernel_ms": ms,
+                         "traffic": None},
             "clocks": clocks.summary(), "e2e": None, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"relative_trace_error": tr_err},
         }), flush=True)

@@ -69,7 +69,7 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
                                       const void *hh_v, const void *hh_tau,
                                       void *q, int64_t ldq);
 
-/* SURVEY.md 8(f) NEXT-1, first version (real FP64 only): bulge chasing of a symmetric band matrix to
+/* SURVEY.md 8(f) NEXT-1, first version: bulge chasing of a symmetric / Hermitian band matrix to
  * tridiagonal form on the device (Eq. 6b; the step is SURVEY.md 8(c) O3 / DESIGN.md
  * R3, R4, R7), emitting the reflectors in the layout the calls above consume.
  *   ab:  DEVICE, (2*nbw+1) x N doubles, column j at ab + j*(2*nbw+1), ab[(i-j) + j*(2*nbw+1)] = B[i][j]
@@ -81,6 +81,10 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
  * chase steps), no host synchronisation, no allocation.  Returns 0; -i for a bad i-th argument
  * (N=1, nbw=2, ab=3, hh_v=4, hh_tau=5, d=6, e=7); > 0 = cudaError_t.  N = 0: no work. */
 int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh_tau,
+                        double *d, double *e, void *stream);
+/* Complex Hermitian (interleaved (re, im); the diagonal of B real): B <- H^H B H with the complex tau
+ * of R2; slot (N-2, 0) is the length-1 phase rotation of R4 that makes T real.  d, e are real. */
+int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau,
                         double *d, double *e, void *stream);
 
 /* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */

@@ -21,7 +21,7 @@ EXPORTS = (
     "elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z",
     "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
-    "elpa2_bulge_chase_d",
+    "elpa2_bulge_chase_d", "elpa2_bulge_chase_z",
 )
 
 
@@ -51,8 +51,9 @@ def lib() -> ctypes.CDLL:
             getattr(L, nm).restype = i32
         L.elpa2_trans_ev_tridi_to_band_host.argtypes = [i32, i64, i32, i64, vp, vp, vp, i64]
         L.elpa2_trans_ev_tridi_to_band_host.restype = i32
-        L.elpa2_bulge_chase_d.argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
-        L.elpa2_bulge_chase_d.restype = i32
+        for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
+            getattr(L, nm).argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
+            getattr(L, nm).restype = i32
         L.elpa2_hh_count.argtypes = [i64, i32]
         L.elpa2_hh_count.restype = i64
         L.elpa2_hh_offset.argtypes = [i64, i32, i64]
@@ -163,20 +164,22 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
 
 
 def bulge_chase(N: int, nbw: int, ab, stream=None):
-    """Band -> tridiagonal on the device (real FP64; Eq. 6b).  ``ab``: CUDA float64 tensor of shape
+    """Band -> tridiagonal on the device (Eq. 6b).  ``ab``: CUDA float64 / complex128 tensor of shape
     (N, 2*nbw+1), row j = column j of the lower band storage (ab[j, i-j] = B[i, j]), overwritten
-    with T.  Returns CUDA tensors (hh_v (G, nbw), hh_tau (G,), d (N,), e (N-1,))."""
+    with T.  Returns CUDA tensors (hh_v (G, nbw), hh_tau (G,), d (N,), e (N-1,)); d, e are real."""
     import torch
 
-    if not ab.is_cuda or ab.dtype != torch.float64 or not ab.is_contiguous() or tuple(ab.shape) != (N, 2 * nbw + 1):
-        raise ValueError("ab must be a contiguous CUDA float64 tensor of shape (N, 2*nbw+1)")
+    if (not ab.is_cuda or ab.dtype not in (torch.float64, torch.complex128) or not ab.is_contiguous()
+            or tuple(ab.shape) != (N, 2 * nbw + 1)):
+        raise ValueError("ab must be a contiguous CUDA float64/complex128 tensor of shape (N, 2*nbw+1)")
     G = hh_count(N, nbw)
-    hh_v = torch.empty((G, nbw), dtype=torch.float64, device=ab.device)
-    hh_tau = torch.empty((G,), dtype=torch.float64, device=ab.device)
+    hh_v = torch.empty((G, nbw), dtype=ab.dtype, device=ab.device)
+    hh_tau = torch.empty((G,), dtype=ab.dtype, device=ab.device)
     d = torch.empty((N,), dtype=torch.float64, device=ab.device)
     e = torch.empty((max(N - 1, 0),), dtype=torch.float64, device=ab.device)
-    rc = lib().elpa2_bulge_chase_d(N, nbw, ab.data_ptr(), hh_v.data_ptr(), hh_tau.data_ptr(), d.data_ptr(),
-                                   e.data_ptr(), _stream_ptr(stream))
+    fn = lib().elpa2_bulge_chase_z if ab.dtype == torch.complex128 else lib().elpa2_bulge_chase_d
+    rc = fn(N, nbw, ab.data_ptr(), hh_v.data_ptr(), hh_tau.data_ptr(), d.data_ptr(), e.data_ptr(),
+            _stream_ptr(stream))
     if rc != 0:
         raise Elpa2BtError(rc)
     return hh_v, hh_tau, d, e

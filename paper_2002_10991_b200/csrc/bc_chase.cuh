@@ -1,5 +1,5 @@
-// bc_chase.cuh -- SURVEY.md 8(f) NEXT-1, first version: bulge chasing of a real symmetric band matrix
-// to tridiagonal form on the GPU (Eq. 6b), emitting the Householder reflectors
+// bc_chase.cuh -- SURVEY.md 8(f) NEXT-1, first version: bulge chasing of a real symmetric (and, further
+// down, complex Hermitian) band matrix to tridiagonal form on the GPU (Eq. 6b), emitting the Householder reflectors
 // directly in the device layout the back-transformation consumes (include/elpa2_bt.h).
 //
 // Step (s, k) -- sweep s, chase block k -- is exactly the oracle's step (R3, R7):
@@ -275,6 +275,144 @@ __global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64
     }
 }
 
+// ---- complex Hermitian version (global-memory step; the tile of a complex step exceeds shared memory) ----
+// Complex arithmetic rounded like C99 without contraction (what the definition's plain loops mean and
+// what the oracle's compiler emits): (a+bi)(c+di) = (ac - bd) + (ad + bc)i with four separately rounded
+// products; 1/(c+di) by Smith's formula, the one libgcc's __divdc3 evaluates for in-range operands.
+struct zc {
+    double re, im;
+};
+__device__ __forceinline__ zc zmul(zc a, zc b)
+{
+    return {__dsub_rn(__dmul_rn(a.re, b.re), __dmul_rn(a.im, b.im)), __dadd_rn(__dmul_rn(a.re, b.im), __dmul_rn(a.im, b.re))};
+}
+__device__ __forceinline__ zc zadd(zc a, zc b) { return {__dadd_rn(a.re, b.re), __dadd_rn(a.im, b.im)}; }
+__device__ __forceinline__ zc zsub(zc a, zc b) { return {__dsub_rn(a.re, b.re), __dsub_rn(a.im, b.im)}; }
+__device__ __forceinline__ zc zconj(zc a) { return {a.re, -a.im}; }
+__device__ __forceinline__ zc zrecip(zc z)        // 1 / z
+{
+    const double c = z.re, d = z.im;
+    if (fabs(c) < fabs(d)) {
+        const double ratio = __ddiv_rn(c, d), denom = __dadd_rn(__dmul_rn(c, ratio), d);
+        return {__ddiv_rn(ratio, denom), __ddiv_rn(-1.0, denom)};
+    }
+    const double ratio = __ddiv_rn(d, c), denom = __dadd_rn(__dmul_rn(d, ratio), c);
+    return {__ddiv_rn(1.0, denom), __ddiv_rn(-ratio, denom)};
+}
+
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t t, int64_t s_hi, zc *__restrict__ ab,
+                                                             zc *__restrict__ hh_v, zc *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    constexpr int64_t ldab = 2 * NBW + 1;
+    __shared__ zc v[NBW], p[NBW], w2[NBW];
+    __shared__ zc s_tau, s_scal;
+    __shared__ double s_beta;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    const int64_t r0 = s + 1 + (k << LG);
+    int64_t r1 = s + ((k + 1) << LG);
+    if (r1 > N - 1) r1 = N - 1;
+    const int L = (int)(r1 - r0 + 1);
+    const int64_t c = (k == 0) ? s : r0 - NBW;
+    const int64_t g = hh_off(N, LG, s) + k;
+#define BC_Z(i, j) ab[((i) - (j)) + (j) * ldab]
+    zc *vout = hh_v + g * NBW;
+    if (k > 0 && L == 1) {
+        for (int i = tid; i < NBW; i += nt) vout[i] = {(i == 0) ? 1.0 : 0.0, 0.0};
+        if (tid == 0) hh_tau[g] = {0.0, 0.0};
+        return;
+    }
+    // --- Householder generator (R2, R7): beta real, tau = ((beta - Re a)/beta, -Im a/beta), v = x/(alpha - beta)
+    if (tid < L) p[tid] = BC_Z(r0 + tid, c);
+    __syncthreads();
+    if (tid == 0) {
+        const double ar = p[0].re, ai = p[0].im;
+        double ss = 0.0;
+        for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dadd_rn(__dmul_rn(p[i].re, p[i].re), __dmul_rn(p[i].im, p[i].im)));
+        if (ss == 0.0 && ai == 0.0) {
+            s_tau = {0.0, 0.0};
+            s_scal = {0.0, 0.0};
+            s_beta = ar;
+        } else {
+            const double nrm = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(ar, ar), __dmul_rn(ai, ai)), ss));
+            const double b = (ar >= 0.0) ? -nrm : nrm;
+            s_tau = {__ddiv_rn(__dsub_rn(b, ar), b), __ddiv_rn(-ai, b)};
+            s_scal = zrecip({__dsub_rn(ar, b), ai});
+            s_beta = b;
+        }
+    }
+    __syncthreads();
+    const zc tau = s_tau, ctau = zconj(s_tau);
+    const bool ident = (tau.re == 0.0 && tau.im == 0.0);
+    for (int i = tid; i < NBW; i += nt) {
+        zc vi = {0.0, 0.0};
+        if (i == 0) vi = {1.0, 0.0};
+        else if (i < L && !ident) vi = zmul(p[i], s_scal);
+        v[i] = vi;
+        vout[i] = vi;
+    }
+    __syncthreads();
+    if (tid < L) BC_Z(r0 + tid, c) = {(tid == 0) ? s_beta : 0.0, 0.0};
+    if (tid == 0) hh_tau[g] = tau;
+    if (ident) return;
+    // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
+    for (int64_t j = c + 1 + tid; j < r0; j += nt) {
+        zc dot = {0.0, 0.0};
+        for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), BC_Z(r0 + i, j)));
+        for (int i = 0; i < L; ++i) BC_Z(r0 + i, j) = zsub(BC_Z(r0 + i, j), zmul(zmul(ctau, v[i]), dot));
+    }
+    // --- (ii) D <- H^H D H: p = v^H D;  M = D - conj(tau) v p;  w2 = M v;  D' = M - tau w2 v^H (lower part)
+    __syncthreads();
+    for (int j = tid; j < L; j += nt) {
+        zc dot = {0.0, 0.0};
+        for (int i = 0; i < L; ++i)
+            dot = zadd(dot, zmul(zconj(v[i]), (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i))));
+        p[j] = dot;
+    }
+    __syncthreads();
+    for (int i = tid; i < L; i += nt) {
+        zc dot = {0.0, 0.0};
+        for (int j = 0; j < L; ++j) {
+            const zc dij = (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i));
+            const zc m = zsub(dij, zmul(zmul(ctau, v[i]), p[j]));
+            dot = zadd(dot, zmul(m, v[j]));
+        }
+        w2[i] = dot;
+    }
+    __syncthreads();
+    for (int j = tid; j < L; j += nt)
+        for (int i = j; i < L; ++i) {
+            const zc m = zsub(BC_Z(r0 + i, r0 + j), zmul(zmul(ctau, v[i]), p[j]));
+            zc r = zsub(m, zmul(zmul(tau, w2[i]), zconj(v[j])));
+            if (i == j) r.im = 0.0;              // a Hermitian diagonal is real
+            BC_Z(r0 + i, r0 + j) = r;
+        }
+    // --- (iii) E <- E H = E - tau (E v) v^H
+    int64_t r2 = r1 + NBW;
+    if (r2 > N - 1) r2 = N - 1;
+    for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
+        zc dot = {0.0, 0.0};
+        for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
+        for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
+    }
+#undef BC_Z
+}
+
+template <int NBW>
+__global__ void bc_extract_kernel_z(int64_t N, const zc *__restrict__ ab, double *__restrict__ d, double *__restrict__ e)
+{
+    constexpr int64_t ldab = 2 * NBW + 1;
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < N) d[i] = ab[i * ldab].re;
+    if (i + 1 < N) e[i] = ab[1 + i * ldab].re;
+}
+
 // d[i] = T[i][i], e[i] = T[i+1][i]
 template <int NBW>
 __global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, double *__restrict__ d, double *__restrict__ e)
@@ -329,6 +467,36 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     }
     if (N >= 1) {
         bc_extract_kernel<NBW><<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ab, d, e);
+        ++nl;
+    }
+    if (launches) *launches = nl;
+    return cudaGetLastError();
+}
+
+// complex: the same wavefronts, global-memory step
+template <int NBW>
+cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double *d, double *e, cudaStream_t st,
+                                 int64_t *launches)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    int64_t nl = 0;
+    if (N >= 2) {
+        const int64_t Kmax = (N - 2 + NBW) >> LG;
+        const int64_t tmax = (3 * (N - 2) > Kmax - 1) ? 3 * (N - 2) : Kmax - 1;
+        for (int64_t t = 0; t <= tmax; ++t) {
+            int64_t s_hi = t / 3;
+            if (s_hi > N - 2) s_hi = N - 2;
+            int64_t s_lo = (t - Kmax + 1 + 2) / 3;
+            if (t - Kmax + 1 <= 0) s_lo = 0;
+            if (s_lo > s_hi) continue;
+            bc_wavefront_kernel_z<NBW><<<(unsigned)(s_hi - s_lo + 1), 128, 0, st>>>(N, t, s_hi, ab, hh_v, hh_tau);
+            ++nl;
+        }
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return e1;
+    }
+    if (N >= 1) {
+        bc_extract_kernel_z<NBW><<<(unsigned)((N + 255) / 256), 256, 0, st>>>(N, ab, d, e);
         ++nl;
     }
     if (launches) *launches = nl;

@@ -275,6 +275,30 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
     return 0;
 }
 
+int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, double *d, double *e, void *stream)
+{
+    if (N < 0) return -1;
+    if (lg_of(nbw) < 0) return -2;
+    g_last_launches = 0;
+    if (N == 0) return 0;
+    if (!ab) return -3;
+    if (N >= 2 && !hh_v) return -4;
+    if (N >= 2 && !hh_tau) return -5;
+    if (!d) return -6;
+    if (N >= 2 && !e) return -7;
+    cudaStream_t st = (cudaStream_t)stream;
+    int64_t nl = 0;
+    cudaError_t err;
+    switch (nbw) {
+    case 32: err = launch_bulge_chase_z<32>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
+    case 64: err = launch_bulge_chase_z<64>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
+    default: err = launch_bulge_chase_z<128>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
+    }
+    if (err != cudaSuccess) return (int)err;
+    g_last_launches = (int)(nl > 0x7fffffff ? 0x7fffffff : nl);
+    return 0;
+}
+
 int64_t elpa2_hh_count(int64_t N, int nbw)
 {
     const int lg = lg_of(nbw);

@@ -28,10 +28,11 @@ def _gpu_chase(ab, N, nbw):
     return hv, ht, d, e, dab
 
 
+@pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("N,nbw", [(2, 32), (3, 32), (33, 32), (34, 32), (100, 32), (65, 64), (200, 64), (515, 64),
                                    (300, 128), (1000, 32), (2500, 64)])
-def test_chase_matches_oracle(N, nbw):
-    ab = si.band_matrix(N, nbw, 500 + N, False)
+def test_chase_matches_oracle(N, nbw, cplx):
+    ab = si.band_matrix(N, nbw, 500 + N, cplx)
     ab_o = ab.copy(order="F")
     hv_o, ht_o, d_o, e_o = orc.bulge_chase(ab_o, nbw)
     hv, ht, d, e, dab = _gpu_chase(ab, N, nbw)
@@ -53,23 +54,25 @@ def test_chase_matches_oracle(N, nbw):
     assert np.abs(t[:, 2:]).max(initial=0.0) <= 1e-12 * scale * max(N, 1)
 
 
+@pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("N,nbw", [(64, 32), (257, 64)])
-def test_chase_eigenvalues_and_end_to_end(N, nbw):
+def test_chase_eigenvalues_and_end_to_end(N, nbw, cplx):
     import torch
     from scipy.linalg import eigh_tridiagonal
 
     from paper_2002_10991_b200 import binding
 
-    ab = si.band_matrix(N, nbw, 77, False)
+    ab = si.band_matrix(N, nbw, 77, cplx)
     B = dense_from_band(ab, nbw)
     hv, ht, d, e, _ = _gpu_chase(ab, N, nbw)
     lam, X = eigh_tridiagonal(d.cpu().numpy(), e.cpu().numpy())
     nB = np.linalg.norm(B, 2)
     assert np.abs(lam - np.linalg.eigvalsh(B)).max() <= 1e-12 * N * nB
     # back-transform the eigenvectors of T with the reflectors that never left the device
-    q = torch.from_numpy(np.ascontiguousarray(X.T)).cuda().t()
+    Xc = X.astype(np.complex128) if cplx else X
+    q = torch.from_numpy(np.ascontiguousarray(Xc.T)).cuda().t()
     binding.trans_ev_tridi_to_band(N, nbw, hv, ht, q)
     torch.cuda.synchronize()
     Y = q.cpu().numpy()
     assert np.abs(B @ Y - Y * lam).max() / nB <= 1e-12 * N
-    assert np.abs(Y.T @ Y - np.eye(N)).max() <= 1e-12 * N
+    assert np.abs(Y.conj().T @ Y - np.eye(N)).max() <= 1e-12 * N
