@@ -54,6 +54,7 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
     if (tid == 0) {
         const double alpha = p[0];
         double ss = 0.0;
+#pragma unroll 8
         for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
         if (ss == 0.0) {
             s_tau = 0.0;
@@ -178,15 +179,18 @@ __global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64
         seg(q, lo, hi);
         if (row >= lo && row < hi) {
             const int64_t j = c + 1 + q;
-            S[q * LDS + row] = ab[(r0 + row - j) + j * ldab];
+            cp_async8(smem_u32(&S[q * LDS + row]), &ab[(r0 + row - j) + j * ldab], 8u);   // all copies in flight at once
         }
     }
+    cp_async_commit();
     if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];       // x = B[r0..r1][c]
+    cp_async_wait_all();
     __syncthreads();
 #define BS(rl, q) S[(q) * LDS + (rl)]
     if (tid == 0) {
         const double alpha = p[0];
         double ss = 0.0;
+#pragma unroll 8
         for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
         if (ss == 0.0) {
             s_tau = 0.0;
