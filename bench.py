@@ -257,6 +257,8 @@ def main() -> None:
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--e2e-steps", type=int, default=2, help="timed host-buffer calls (0 = skip)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],
+                    help="library variant for A/B runs (include/elpa2_bt.h): 0 default, 2 register window, 3 two chains per pass")
     ap.add_argument("--chase", action="store_true",
                     help="time SURVEY 8(f) NEXT-1 instead: the GPU bulge chase (real configs) that produces the reflectors")
     ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",
@@ -306,6 +308,7 @@ def main() -> None:
     hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
     q = si.gaussian_block(N, nev, seed_x + 7919 * rank, cplx, "cuda")
     stream = torch.cuda.current_stream()
+    binding.set_variant(args.variant)
 
     def step():
         binding.trans_ev_tridi_to_band(N, nbw, hh_v, hh_tau, q, stream=stream)
@@ -397,7 +400,8 @@ def main() -> None:
                        "l2": ("inputs larger than L2 (%.2f GiB of q + reflectors per step)"
                               % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
                              else "inputs smaller than L2; config is latency-bound (DESIGN.md)",
-                       "parallelism": "column shards, no collective" if world > 1 else "single GPU"},
+                       "parallelism": "column shards, no collective" if world > 1 else "single GPU",
+                       "variant": args.variant},
             "roofline": {"bound": "tensor" if tensor_path else "alu", "achieved": achieved, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved / peak_tf,
                          "peak_source": ("FP64 %s probe measured in this run (elpa2_bt_probe_fp64 kind %d); "

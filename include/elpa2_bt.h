@@ -99,8 +99,10 @@ int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
  * aggregation of 8 reflectors on the FP64 tensor cores, R6: a T-factor prepass kernel + the main
  * kernel = 2 launches; its scratch comes from a stream-ordered pool that keeps its memory),
  * 1 = plain kernel (one thread per column, literal reverse generation order), 2 = one reflector at
- * a time in a register-resident window (DFMA, 1 launch).  Returns the previous variant or -1 if
- * `variant` is unknown. */
+ * a time in a register-resident window (DFMA, 1 launch), 3 = the default path with two chains per
+ * pass (real only: pairs of warps share their columns and walk alternate chains, handing rows over
+ * through L2 -- half the DRAM traffic, about 8 % slower; complex runs variant 0).  Returns the
+ * previous variant or -1 if `variant` is unknown. */
 int elpa2_bt_last_launch_count(void);
 int elpa2_bt_set_variant(int variant);
 

@@ -246,8 +246,8 @@ __device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool co
 
 // ---- a warp with NG slabs of 8 columns ---------------------------------------------------------------
 // CP = false: the 8 warps of a CTA share one ring and walk every chain (grp = 0, member = warp).
-// CP = true (NG = 1): a.P warps share a slab; warp (grp, member) walks chains grp, grp+P, .. of slab
-// `slab`; the warps with the same grp share ring grp (NS/P stages) and are its `nmem` members.
+// CP = true: a.P warps share NG slabs; warp (grp, member) walks chains grp, grp+P, .. of the slabs
+// starting at `slab`; the warps with the same grp share ring grp (NS/P stages) and are its `nmem` members.
 template <class C, int NG, bool CP>
 __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int lane, const int grp,
                                            const int member, const int nmem, const int64_t col0, const int64_t slab)
@@ -465,7 +465,8 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
     const int64_t nslab = (a.nev + 7) >> 3;
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
-    const int nact = nmine < NW ? nmine : NW;          // members of a ring (P = 1: active warps)
+    const int nslot = NW / (a.P > 1 ? a.P : 1);
+    const int nact = nmine < nslot ? nmine : nslot;    // members of a ring (P = 1: active warps)
 
     // the ring starts as zeros: the skew padding of VA / VB is never written by the copies, and
     // positions of reflectors outside a chain keep finite values (their row and column of T are 0)
@@ -481,9 +482,20 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
     __syncthreads();
 
     if (a.P > 1) {
-        const int grp = warp % a.P, member = warp / a.P;
-        if (member >= nmine) return;
-        wy_consume<C, 1, true>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
+        // chain-parallel: `member` = the a.P warps that share slabs; member slots NW / P
+        const int grp = warp % a.P, member = warp / a.P, nm = NW / a.P;
+        const int base = nmine / nm, extra = nmine % nm;
+        const int ng = base + (member < extra ? 1 : 0);
+        const int64_t wslab0 = slab0 + (int64_t)member * base + (member < extra ? member : extra);
+        if (ng == 0) return;
+        if (NGMAX >= 4 && ng == 4)
+            wy_consume<C, (NGMAX >= 4 ? 4 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+        else if (NGMAX >= 3 && ng == 3)
+            wy_consume<C, (NGMAX >= 3 ? 3 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+        else if (ng == 2)
+            wy_consume<C, 2, true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+        else
+            wy_consume<C, 1, true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         return;
     }
     const int base = nmine / NW, extra = nmine % NW;
@@ -551,7 +563,7 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     wy_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
+    const int64_t per_cta = (int64_t)(C::NW / P) * C::NGMAX;
     const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
     int64_t grid = nsm * waves;                       // a multiple of the SM count ...
     if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that

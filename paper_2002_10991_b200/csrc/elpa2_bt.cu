@@ -109,14 +109,14 @@ cudaMemPool_t scratch_pool(cudaError_t *err)
 
 template <int NBW>
 cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                   int align16, cudaStream_t st)
+                   int align16, cudaStream_t st, int force_P = 0)
 {
     cudaError_t e;
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
     if ((e = cudaMallocFromPoolAsync(&tn, wy_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
-    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), tn, st);
+    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), tn, st, force_P);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
@@ -160,19 +160,21 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
         const unsigned grid = (unsigned)((nev + 127) / 128);
         bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
         e = cudaGetLastError();
-    } else if (g_variant == 0 && CPLX) {
+    } else if ((g_variant == 0 || g_variant == 3) && CPLX) {
         switch (nbw) {
         case 32: e = run_wyz<32>(N, nev, hh_v, hh_tau, q, ldq, st); break;
         case 64: e = run_wyz<64>(N, nev, hh_v, hh_tau, q, ldq, st); break;
         default: e = run_wyz<128>(N, nev, hh_v, hh_tau, q, ldq, st); break;
         }
         nlaunch = 2;
-    } else if (g_variant == 0) {
+    } else if (g_variant == 0 || (g_variant == 3 && !CPLX)) {
+        // variant 3: two chains per pass (pairs of warps share their slabs, hand-over through L2)
         const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
+        const int fp = (g_variant == 3 && wy_nchains(N, lg) >= 8) ? 2 : 0;
         switch (nbw) {
-        case 32: e = run_wy<32>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        case 64: e = run_wy<64>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
-        default: e = run_wy<128>(N, nev, hh_v, hh_tau, q, ldq, align16, st); break;
+        case 32: e = run_wy<32>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
+        case 64: e = run_wy<64>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
+        default: e = run_wy<128>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
         }
         nlaunch = 2;
     } else {
@@ -324,7 +326,7 @@ int elpa2_bt_last_launch_count(void) { return g_last_launches; }
 
 int elpa2_bt_set_variant(int variant)
 {
-    if (variant < 0 || variant > 2) return -1;
+    if (variant < 0 || variant > 3) return -1;
     const int old = g_variant;
     g_variant = variant;
     return old;

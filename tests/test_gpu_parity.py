@@ -149,6 +149,14 @@ def test_register_window_variant_matches_oracle(nbw, cplx):
     _check(2 * nbw + 9, nbw, 19, cplx, ldq=2 * nbw + 9 + 3, variant=2)
 
 
+@pytest.mark.parametrize("nbw", [32, 64, 128])
+def test_two_chains_per_pass_variant(nbw):
+    # variant 3 (real): pairs of warps share their slabs and walk alternate chains, several slabs per warp
+    _check(9 * nbw + 3, nbw, 148 * 8 * 2 + 21, False, variant=3)     # 2-3 slabs per CTA
+    _check(8 * nbw, nbw, 5000, False, variant=3)
+    _check(3 * nbw + 5, nbw, 100, False, variant=3)                  # too few chains: falls back to P = 1
+
+
 def test_degenerate_no_work():
     for N, nev in ((0, 5), (1, 5), (40, 0)):
         x = np.zeros((N, nev), order="F")
