@@ -36,16 +36,16 @@
 
 namespace elpa2bt {
 
-template <int NBW_>
+template <int NBW_, int NW_ = 8>
 struct WyCfg {
     static constexpr int NBW = NBW_;
     static constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     static constexpr int NT = NBW / 8 + 1;            // 8-row tiles in the window
     static constexpr int W = 8 * NT;                  // window rows (= nbw + 8; W % 16 == 8)
-    static constexpr int NW = 8;                      // warps per CTA
-    static constexpr int NGMAX = (NBW <= 64) ? 4 : 2; // most 8-column slabs per warp
-    static constexpr int NS = 8;                      // ring stages
-    static constexpr int LGNS = 3;
+    static constexpr int NW = NW_;                    // warps per CTA: 8 (255 registers) or, for few columns, 16 (128)
+    static constexpr int NGMAX = (NW_ > 8) ? 1 : (NBW <= 64) ? 4 : 2;   // most 8-column slabs per warp
+    static constexpr int NS = (NW_ > 8) ? 16 : 8;     // ring stages
+    static constexpr int LGNS = (NW_ > 8) ? 4 : 3;
     static constexpr int LAG = 4;                     // staging waits for the block LAG iterations back
     static constexpr int VA_OFF = 0;                  // VA[i][w] = V, row stride W
     static constexpr int YB_OFF = 8 * W;              // YB[w][j] = (V (-T))[w][j], row stride 8
@@ -255,7 +255,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     constexpr int NT = C::NT, W = C::W, NBW = C::NBW;
     constexpr int NACC = (NG >= 3) ? 1 : 2;          // dot-product accumulator sets per slab
     const int P = CP ? a.P : 1;
-    const int lgs = CP ? (P == 2 ? C::LGNS - 1 : C::LGNS - 2) : C::LGNS;   // log2(stages of this ring)
+    const int lgs = CP ? (P == 2 ? C::LGNS - 1 : C::LGNS - 2) : C::LGNS;   // log2(stages of this ring), P <= 4
     const int NSP = 1 << lgs, LAG = NSP >> 1;
     double *ring = reinterpret_cast<double *>(smem) + (size_t)grp * NSP * C::STAGE_DOUBLES;
     const uint32_t bar_full = smem_u32(smem + C::OFF_BAR) + 8 * grp * NSP;
@@ -451,10 +451,10 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
 //  P = 1: at most NW*NGMAX slabs per CTA; warp w takes n/NW of them, +1 for the first n%NW warps
 //         (warps w and w+4 share a sub-partition, so the extras land on different sub-partitions first).
 //  P > 1 (few slabs): at most NW/P slabs per CTA; warp w works on slab w/P, chains (w%P) + m P.
-template <int NBW>
-__global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
+template <int NBW, int NWARPS>
+__global__ void __launch_bounds__(NWARPS * 32, 1) bt_wy_kernel(const WyArgs a)
 {
-    using C = WyCfg<NBW>;
+    using C = WyCfg<NBW, NWARPS>;
     constexpr int NS = C::NS, NW = C::NW, NGMAX = C::NGMAX;
     extern __shared__ __align__(128) unsigned char smem[];
     double *ring = reinterpret_cast<double *>(smem);
@@ -492,12 +492,13 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
             wy_consume<C, (NGMAX >= 4 ? 4 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         else if (NGMAX >= 3 && ng == 3)
             wy_consume<C, (NGMAX >= 3 ? 3 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
-        else if (ng == 2)
-            wy_consume<C, 2, true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+        else if (NGMAX >= 2 && ng == 2)
+            wy_consume<C, (NGMAX >= 2 ? 2 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         else
             wy_consume<C, 1, true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         return;
     }
+    if (NWARPS > 8) return;                            // the 16-warp build is chain-parallel only
     const int base = nmine / NW, extra = nmine % NW;
     const int ng = base + (warp < extra ? 1 : 0);
     const int64_t wslab0 = slab0 + (int64_t)warp * base + (warp < extra ? warp : extra);
@@ -507,9 +508,9 @@ __global__ void __launch_bounds__(256, 1) bt_wy_kernel(const WyArgs a)
         wy_consume<C, (NGMAX >= 4 ? 4 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (NGMAX >= 3 && ng == 3)
         wy_consume<C, (NGMAX >= 3 ? 3 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
-    else if (ng == 2)
-        wy_consume<C, 2, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
-    else
+    else if (NGMAX >= 2 && ng == 2)
+        wy_consume<C, (NGMAX >= 2 ? 2 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+    else if (NWARPS <= 8)
         wy_consume<C, 1, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
 }
 
@@ -537,23 +538,38 @@ size_t wy_scratch_bytes(int64_t N, int64_t nev)
     return wy_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
-template <int NBW>
-cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                      int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0)
+template <int NBW, int NWARPS>
+cudaError_t launch_wy_main(const WyArgs &a, int64_t nslab, int nsm, cudaStream_t st)
 {
-    using C = WyCfg<NBW>;
-    auto kern = bt_wy_kernel<NBW>;
+    using C = WyCfg<NBW, NWARPS>;
+    auto kern = bt_wy_kernel<NBW, NWARPS>;
     static bool attr_done = false;
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
+    const int64_t per_cta = (int64_t)(C::NW / a.P) * C::NGMAX;
+    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
+    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
+    if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that
+    kern<<<(unsigned)grid, NWARPS * 32, C::SMEM_BYTES, st>>>(a);
+    return cudaGetLastError();
+}
+
+// force_P > 0 overrides the number of warps per slab of the 8-warp kernel; force_nw = 8 keeps the
+// 16-warp kernel (few columns: 4 warps per slab, 128 registers each) from being chosen.
+template <int NBW>
+cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
+                      int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0, int force_nw = 0)
+{
+    using C = WyCfg<NBW>;
     const int64_t K0 = wy_nchains(N, C::LG);
     const int64_t nslab = (nev + 7) >> 3;
     double *tn = (double *)scratch;
     uint32_t *prog = (uint32_t *)((char *)scratch + wy_tn_bytes<NBW>(N));
-    const int P = force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 4);
+    const bool many_warps = NBW <= 64 && force_P == 0 && force_nw != 8 && nslab <= (int64_t)nsm * 4 && K0 >= 16;
+    const int P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 4));
     cudaError_t e;
     if (P > 1) {
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
@@ -563,10 +579,6 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     wy_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const int64_t per_cta = (int64_t)(C::NW / P) * C::NGMAX;
-    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
-    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
-    if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that
     WyArgs a;
     a.N = N;
     a.nev = nev;
@@ -578,8 +590,8 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     a.prog = prog;
     a.align16 = align16;
     a.P = P;
-    kern<<<(unsigned)grid, 256, C::SMEM_BYTES, st>>>(a);
-    return cudaGetLastError();
+    if (many_warps) return launch_wy_main<(NBW <= 64 ? NBW : 64), 16>(a, nslab, nsm, st);
+    return launch_wy_main<NBW, 8>(a, nslab, nsm, st);
 }
 
 }  // namespace elpa2bt
