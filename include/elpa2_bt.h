@@ -106,6 +106,12 @@ int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
 int elpa2_bt_last_launch_count(void);
 int elpa2_bt_set_variant(int variant);
 
+/* Launch plan of the default variant's main kernel for a problem on a device with n_sm SMs (host, pure
+ * integer arithmetic, no device needed; DESIGN.md 5.1 "Decomposition"): out = { CTAs, warps per CTA,
+ * warps per slab group P (= chains walked per pass), slabs of 8 columns, most slabs per CTA, bytes
+ * of scratch }.  All zero when there is no work.  Returns 0 or -i for a bad i-th argument. */
+int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int64_t out[6]);
+
 const char *elpa2_bt_version(void);
 
 /* Measurement aid (synchronous; allocates and frees a small device buffer): sustained FP64 ALU

@@ -525,6 +525,32 @@ inline int wy_pick_P(int64_t nslab, int64_t K0, int nsm, int nw, int maxP)
     return nslab <= (int64_t)nsm * nw ? P : 1;
 }
 
+// launch plan of the main kernel (pure host arithmetic; exported as elpa2_bt_plan for the CPU tests)
+struct WyPlan {
+    int64_t grid;        // CTAs
+    int nwarps;          // warps per CTA: 8, or 16 (real, few columns)
+    int P;               // warps per slab group (chains per pass)
+    int64_t nslab;       // slabs of 8 columns
+    int64_t per_cta;     // most slabs a CTA can take
+};
+inline WyPlan wy_plan(bool cplx, int nbw, int64_t N, int64_t nev, int nsm, int force_P, int force_nw)
+{
+    const int lg = nbw == 32 ? 5 : nbw == 64 ? 6 : 7;
+    const int64_t K0 = wy_nchains(N, lg);
+    WyPlan pl;
+    pl.nslab = (nev + 7) >> 3;
+    const int ngmax8 = cplx ? (nbw <= 64 ? 2 : 1) : (nbw <= 64 ? 4 : 2);
+    const bool many_warps = !cplx && nbw <= 64 && force_P == 0 && force_nw != 8 && pl.nslab <= (int64_t)nsm * 4 && K0 >= 16;
+    pl.nwarps = many_warps ? 16 : 8;
+    pl.P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(pl.nslab, K0, nsm, 8, cplx ? 2 : 4));
+    // (the complex kernel and the 16-warp build walk one slab per warp in chain-parallel mode)
+    pl.per_cta = (int64_t)(pl.nwarps / pl.P) * ((many_warps || (cplx && pl.P > 1)) ? 1 : ngmax8);
+    const int64_t waves = (pl.nslab + nsm * pl.per_cta - 1) / (nsm * pl.per_cta);
+    pl.grid = nsm * waves;                            // a multiple of the SM count ...
+    if (pl.grid > pl.nslab) pl.grid = pl.nslab;       // ... unless there are fewer slabs than that
+    return pl;
+}
+
 // bytes of scratch the two kernels share: -T factors, then the chain-progress counters
 template <int NBW>
 size_t wy_tn_bytes(int64_t N)
@@ -539,7 +565,7 @@ size_t wy_scratch_bytes(int64_t N, int64_t nev)
 }
 
 template <int NBW, int NWARPS>
-cudaError_t launch_wy_main(const WyArgs &a, int64_t nslab, int nsm, cudaStream_t st)
+cudaError_t launch_wy_main(const WyArgs &a, const WyPlan &pl, cudaStream_t st)
 {
     using C = WyCfg<NBW, NWARPS>;
     auto kern = bt_wy_kernel<NBW, NWARPS>;
@@ -549,11 +575,7 @@ cudaError_t launch_wy_main(const WyArgs &a, int64_t nslab, int nsm, cudaStream_t
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int64_t per_cta = (int64_t)(C::NW / a.P) * C::NGMAX;
-    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
-    int64_t grid = nsm * waves;                       // a multiple of the SM count ...
-    if (grid > nslab) grid = nslab;                   // ... unless there are fewer slabs than that
-    kern<<<(unsigned)grid, NWARPS * 32, C::SMEM_BYTES, st>>>(a);
+    kern<<<(unsigned)pl.grid, NWARPS * 32, C::SMEM_BYTES, st>>>(a);
     return cudaGetLastError();
 }
 
@@ -568,8 +590,8 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     const int64_t nslab = (nev + 7) >> 3;
     double *tn = (double *)scratch;
     uint32_t *prog = (uint32_t *)((char *)scratch + wy_tn_bytes<NBW>(N));
-    const bool many_warps = NBW <= 64 && force_P == 0 && force_nw != 8 && nslab <= (int64_t)nsm * 4 && K0 >= 16;
-    const int P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 4));
+    const WyPlan pl = wy_plan(false, NBW, N, nev, nsm, force_P, force_nw);
+    const int P = pl.P;
     cudaError_t e;
     if (P > 1) {
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
@@ -590,8 +612,8 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     a.prog = prog;
     a.align16 = align16;
     a.P = P;
-    if (many_warps) return launch_wy_main<(NBW <= 64 ? NBW : 64), 16>(a, nslab, nsm, st);
-    return launch_wy_main<NBW, 8>(a, nslab, nsm, st);
+    if (pl.nwarps == 16) return launch_wy_main<(NBW <= 64 ? NBW : 64), 16>(a, pl, st);
+    return launch_wy_main<NBW, 8>(a, pl, st);
 }
 
 }  // namespace elpa2bt

@@ -462,7 +462,8 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
     const int64_t nslab = (nev + 7) >> 3;
     double *tn_scratch = (double *)scratch;
     uint32_t *prog = (uint32_t *)((char *)scratch + wyz_tn_bytes<NBW>(N));
-    const int P = force_P > 0 ? force_P : wy_pick_P(nslab, K0, nsm, C::NW, 2);
+    const WyPlan pl = wy_plan(true, NBW, N, nev, nsm, force_P, 8);
+    const int P = pl.P;
     cudaError_t e;
     if (P > 1) {
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
@@ -472,10 +473,7 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
     wyz_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    const int64_t per_cta = P > 1 ? C::NW / P : (int64_t)C::NW * C::NGMAX;
-    const int64_t waves = (nslab + nsm * per_cta - 1) / (nsm * per_cta);
-    int64_t grid = nsm * waves;
-    if (grid > nslab) grid = nslab;
+    const int64_t grid = pl.grid;
     WyArgs a;
     a.N = N;
     a.nev = nev;

@@ -322,6 +322,32 @@ int elpa2_hh_blocks(int64_t N, int nbw, int64_t s)
     return (int)((N - 1 - s + nbw - 1) >> lg);
 }
 
+int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int64_t out[6])
+{
+    const int lg = lg_of(nbw);
+    if (N < 0) return -2;
+    if (lg < 0) return -3;
+    if (nev < 0) return -4;
+    if (n_sm < 1) return -5;
+    if (!out) return -6;
+    for (int i = 0; i < 6; ++i) out[i] = 0;
+    if (N <= 1 || nev == 0) return 0;
+    const int fp = (g_variant == 3 && !is_complex && wy_nchains(N, lg) >= 8) ? 2 : 0;
+    const WyPlan pl = wy_plan(is_complex != 0, nbw, N, nev, n_sm, fp, is_complex ? 8 : 0);
+    size_t scratch = 0;
+    if (is_complex)
+        scratch = nbw == 32 ? wyz_scratch_bytes<32>(N, nev) : nbw == 64 ? wyz_scratch_bytes<64>(N, nev) : wyz_scratch_bytes<128>(N, nev);
+    else
+        scratch = nbw == 32 ? wy_scratch_bytes<32>(N, nev) : nbw == 64 ? wy_scratch_bytes<64>(N, nev) : wy_scratch_bytes<128>(N, nev);
+    out[0] = pl.grid;
+    out[1] = pl.nwarps;
+    out[2] = pl.P;
+    out[3] = pl.nslab;
+    out[4] = pl.per_cta;
+    out[5] = (int64_t)scratch;
+    return 0;
+}
+
 int elpa2_bt_last_launch_count(void) { return g_last_launches; }
 
 int elpa2_bt_set_variant(int variant)

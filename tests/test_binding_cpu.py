@@ -94,3 +94,36 @@ def test_missing_library_raises(monkeypatch):
     monkeypatch.setattr(binding, "LIB_PATH", "/nonexistent/libelpa2_bt.so")
     with pytest.raises(RuntimeError, match="no CPU fallback"):
         binding.lib()
+
+
+def test_launch_plan_of_the_five_configs():
+    """elpa2_bt_plan: host arithmetic of the decomposition, no device needed."""
+    want = {
+        (False, 512, 32, 512): (64, 16, 4),          # 64 slabs: one per CTA, 4 warps on each
+        (False, 4096, 64, 4096): (148, 16, 4),       # 512 slabs: 3-4 per CTA, 16-warp build
+        (True, 8192, 64, 4096): (148, 8, 2),         # complex: 8 warps, 2 per slab
+        (False, 32768, 64, 32768): (148, 8, 1),      # 4096 slabs: 27-28 per CTA
+        (True, 16384, 128, 8192): (148, 8, 1),       # 1024 slabs: 6-7 per CTA
+    }
+    for (cplx, N, nbw, nev), (grid, nw, P) in want.items():
+        pl = binding.plan(cplx, N, nbw, nev, 148)
+        assert (pl["grid"], pl["warps_per_cta"], pl["P"]) == (grid, nw, P), (cplx, N, nbw, nev, pl)
+        assert pl["slabs"] == (nev + 7) // 8
+
+
+def test_launch_plan_invariants():
+    import itertools
+
+    for cplx, nbw, N, nev, nsm in itertools.product((False, True), (32, 64, 128), (2, 70, 600, 5000),
+                                                    (1, 8, 9, 1000, 9473, 40000, 100001), (1, 7, 148)):
+        pl = binding.plan(cplx, N, nbw, nev, nsm)
+        nslab = (nev + 7) // 8
+        assert pl["slabs"] == nslab
+        assert 1 <= pl["grid"] <= max(nslab, 1)
+        assert pl["grid"] == nslab or pl["grid"] % nsm == 0          # a multiple of the SM count, or one slab per CTA
+        assert pl["P"] in (1, 2, 4) and pl["warps_per_cta"] in (8, 16) and pl["warps_per_cta"] % pl["P"] == 0
+        # every slab has a place: the fullest CTA gets ceil(nslab / grid) slabs
+        assert -(-nslab // pl["grid"]) <= pl["slabs_per_cta_max"], (cplx, nbw, N, nev, nsm, pl)
+        assert pl["scratch_bytes"] > 0
+    assert binding.plan(False, 1, 64, 10) == dict.fromkeys(("grid", "warps_per_cta", "P", "slabs", "slabs_per_cta_max",
+                                                           "scratch_bytes"), 0)
