@@ -126,22 +126,14 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
 // copies those segments into a tile S[col][row - r0] (column stride odd: conflict-free both ways),
 // runs the step there with exactly the arithmetic of bc_wavefront_kernel, and copies them back.
 template <int NBW>
-__global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64_t t, int64_t s_hi,
-                                                                double *__restrict__ ab, double *__restrict__ hh_v,
-                                                                double *__restrict__ hh_tau)
+__device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
+                                             double *__restrict__ hh_v, double *__restrict__ hh_tau, double *S, double *v,
+                                             double *p, double *w2, double *sc)
 {
     constexpr int LG = (NBW == 32) ? 5 : 6;
     constexpr int64_t ldab = 2 * NBW + 1;
     constexpr int LDS = 2 * NBW + 1;              // tile column stride (doubles)
-    extern __shared__ double S[];                 // (2 NBW - 1) columns x LDS
-    __shared__ double v[NBW], p[NBW], w2[NBW];
-    __shared__ double s_tau, s_scal, s_beta;
     const int tid = threadIdx.x, nt = blockDim.x;
-    const int64_t s = s_hi - blockIdx.x;
-    if (s < 0) return;
-    const int64_t k = t - 3 * s;
-    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
-    if (k < 0 || k >= K) return;
     const int64_t r0 = s + 1 + (k << LG);
     int64_t r1 = s + ((k + 1) << LG);
     if (r1 > N - 1) r1 = N - 1;
@@ -193,25 +185,25 @@ __global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64
 #pragma unroll 8
         for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
         if (ss == 0.0) {
-            s_tau = 0.0;
-            s_scal = 0.0;
-            s_beta = alpha;
+            sc[0] = 0.0;
+            sc[1] = 0.0;
+            sc[2] = alpha;
         } else {
             const double nrm = sqrt(__dadd_rn(__dmul_rn(alpha, alpha), ss));
             const double b = (alpha >= 0.0) ? -nrm : nrm;
-            s_tau = __ddiv_rn(__dsub_rn(b, alpha), b);
-            s_scal = __ddiv_rn(1.0, __dsub_rn(alpha, b));
-            s_beta = b;
+            sc[0] = __ddiv_rn(__dsub_rn(b, alpha), b);
+            sc[1] = __ddiv_rn(1.0, __dsub_rn(alpha, b));
+            sc[2] = b;
         }
     }
     __syncthreads();
-    const double tau = s_tau;
+    const double tau = sc[0];
     for (int i = tid; i < NBW; i += nt) {
-        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], s_scal) : 0.0);
+        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], sc[1]) : 0.0);
         v[i] = vi;
         vout[i] = vi;
     }
-    if (tid < L) ab[(r0 + tid - c) + c * ldab] = (tid == 0) ? s_beta : 0.0;
+    if (tid < L) ab[(r0 + tid - c) + c * ldab] = (tid == 0) ? sc[2] : 0.0;
     if (tid == 0) hh_tau[g] = tau;
     __syncthreads();
     if (tau == 0.0) return;                       // the tile is unchanged: nothing to copy back
@@ -275,6 +267,58 @@ __global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64
         if (row >= lo && row < hi) {
             const int64_t j = c + 1 + q;
             ab[(r0 + row - j) + j * ldab] = S[q * LDS + row];
+        }
+    }
+}
+
+// one launch per wavefront t = 3s + k
+template <int NBW>
+__global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64_t t, int64_t s_hi,
+                                                                double *__restrict__ ab, double *__restrict__ hh_v,
+                                                                double *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : 6;
+    extern __shared__ double S[];                 // (2 NBW - 1) columns x (2 NBW + 1)
+    __shared__ double v[NBW], p[NBW], w2[NBW], sc[3];
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc);
+}
+
+// persistent version: one CTA per SM, CTA c walks sweeps c, c + grid, ...; step (s, k) waits until sweep s-1
+// has finished step k+2 (or all of its steps): prog[s] = steps of sweep s finished, published with a
+// gpu-scope release after the CTA's stores, polled with gpu-scope acquire loads (which also drop the
+// SM's L1 lines, so the staging copies read what the other SM wrote).  No wavefront barrier, no launch
+// per wavefront; the dependency chain (3 steps per sweep) is what remains.
+template <int NBW>
+__global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *__restrict__ ab, double *__restrict__ hh_v,
+                                                            double *__restrict__ hh_tau, uint32_t *__restrict__ prog)
+{
+    constexpr int LG = (NBW == 32) ? 5 : 6;
+    extern __shared__ double S[];
+    __shared__ double v[NBW], p[NBW], w2[NBW], sc[3];
+    const int tid = threadIdx.x;
+    for (int64_t s = blockIdx.x; s <= N - 2; s += gridDim.x) {
+        const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+        const int64_t Kprev = (N - s + NBW - 1) >> LG;      // K(s-1)
+        uint32_t known = 0;
+        for (int64_t k = 0; k < K; ++k) {
+            if (s > 0) {
+                const uint32_t need = (uint32_t)((k + 3 < Kprev) ? k + 3 : Kprev);
+                if (tid == 0) {
+                    while (known < need) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(prog + s - 1) : "memory");
+                    }
+                }
+                __syncthreads();
+            }
+            bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc);
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(prog + s), "r"((uint32_t)(k + 1)) : "memory");
         }
     }
 }
@@ -427,10 +471,11 @@ __global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, doub
     if (i + 1 < N) e[i] = ab[1 + i * ldab];
 }
 
-// host: all wavefronts t = 3s + k, in order, on one stream.  *launches = kernels launched.
+// host: prog == nullptr (or nbw = 128): all wavefronts t = 3s + k, in order, on one stream;
+// otherwise the persistent kernel (prog: N zeroed counters).  *launches = kernels launched.
 template <int NBW>
 cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_tau, double *d, double *e,
-                               cudaStream_t st, int64_t *launches)
+                               cudaStream_t st, int64_t *launches, uint32_t *prog = nullptr, int nsm = 0)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     int64_t nl = 0;
@@ -444,7 +489,22 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
             attr_done = true;
         }
     }
-    if (N >= 2) {
+    if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
+        auto pk = bc_persistent_kernel<(NBW <= 64 ? NBW : 64)>;
+        static bool pattr_done = false;
+        if (!pattr_done) {
+            cudaError_t e0 = cudaFuncSetAttribute(pk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
+            if (e0 != cudaSuccess) return e0;
+            pattr_done = true;
+        }
+        // one CTA per SM (its tile takes more than half of an SM's shared memory): all CTAs are resident,
+        // which the flag waits between sweeps rely on
+        const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
+        pk<<<(unsigned)grid, 256, smem_bytes, st>>>(N, ab, hh_v, hh_tau, prog);
+        ++nl;
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return e1;
+    } else if (N >= 2) {
         const int64_t Kmax = (N - 2 + NBW) >> LG;                  // K(0)
         // last wavefront: max over s of 3s + K(s) - 1; K(s) >= 1 for s <= N-2, so s = N-2 gives 3(N-2)
         int64_t tmax = 0;
