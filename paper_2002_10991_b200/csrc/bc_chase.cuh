@@ -128,7 +128,8 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
 template <int NBW>
 __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
                                              double *__restrict__ hh_v, double *__restrict__ hh_tau, double *S, double *v,
-                                             double *p, double *w2, double *sc)
+                                             double *p, double *w2, double *sc, uint32_t *head_mine = nullptr,
+                                             const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
 {
     constexpr int LG = (NBW == 32) ? 5 : 6;
     constexpr int64_t ldab = 2 * NBW + 1;
@@ -143,7 +144,10 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
     double *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {
         for (int i = tid; i < NBW; i += nt) vout[i] = (i == 0) ? 1.0 : 0.0;
-        if (tid == 0) hh_tau[g] = 0.0;
+        if (tid == 0) {
+            hh_tau[g] = 0.0;
+            if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+        }
         return;
     }
     int64_t r2 = r1 + NBW;
@@ -204,7 +208,11 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
         vout[i] = vi;
     }
     if (tid < L) ab[(r0 + tid - c) + c * ldab] = (tid == 0) ? sc[2] : 0.0;
-    if (tid == 0) hh_tau[g] = tau;
+    if (tid == 0) {
+        hh_tau[g] = tau;
+        // persistent mode: the head element (beta) is all the next sweep's step (s+1, k-2) still lacks
+        if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+    }
     __syncthreads();
     if (tau == 0.0) return;                       // the tile is unchanged: nothing to copy back
     // Blocks (i), (ii), (iii) are disjoint and only read v: three groups of 64 threads run them side by
@@ -222,6 +230,16 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
     } else if (grp == 1) {
         // --- (iii): one thread per row L .. nR-1
         for (int rl = L + t64; rl < nR; rl += 64) {
+            if (need_head && rl == nR - 1) {
+                // the corner (last row, last column) is the head element of step (s-1, k+2), which may be
+                // running right now: wait until it has written beta there, then fetch it
+                uint32_t h;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                } while (h < need_head);
+                const int64_t jc = c + 1 + (nA + L - 1);
+                BS(rl, nA + L - 1) = __ldcg(&ab[(r0 + rl - jc) + jc * ldab]);
+            }
             double dot = 0.0;
 #pragma unroll 8
             for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BS(rl, nA + l), v[l]));
@@ -288,11 +306,14 @@ __global__ void __launch_bounds__(256) bc_wavefront_smem_kernel(int64_t N, int64
     bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc);
 }
 
-// persistent version: one CTA per SM, CTA c walks sweeps c, c + grid, ...; step (s, k) waits until sweep s-1
-// has finished step k+2 (or all of its steps): prog[s] = steps of sweep s finished, published with a
-// gpu-scope release after the CTA's stores, polled with gpu-scope acquire loads (which also drop the
-// SM's L1 lines, so the staging copies read what the other SM wrote).  No wavefront barrier, no launch
-// per wavefront; the dependency chain (3 steps per sweep) is what remains.
+// persistent version: one CTA per SM, CTA c walks sweeps c, c + grid, ...  Step (s, k) overlaps step
+// (s-1, k+2) in ONE element only -- the head element of (s-1, k+2) is the corner (last row, last column)
+// of (s, k)'s block below -- so (s, k) starts as soon as (s-1, k+1) is finished (done[s-1] >= k+2) and
+// only the thread that owns the last row of the block below waits for head[s-1] >= k+3, i.e. for
+// (s-1, k+2) to have written its beta (which it does first thing, after reading the old value: no
+// write-after-read hazard either).  The dependency chain is 2 steps per sweep instead of 3.  Flags are
+// published with gpu-scope releases after the stores they cover and polled with gpu-scope acquires
+// (which also drop the SM's L1 lines, so the staging copies read what the other SM wrote).
 template <int NBW>
 __global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *__restrict__ ab, double *__restrict__ hh_v,
                                                             double *__restrict__ hh_tau, uint32_t *__restrict__ prog)
@@ -301,24 +322,28 @@ __global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *_
     extern __shared__ double S[];
     __shared__ double v[NBW], p[NBW], w2[NBW], sc[3];
     const int tid = threadIdx.x;
+    uint32_t *done = prog, *head = prog + N;          // steps finished / steps whose head element is written
     for (int64_t s = blockIdx.x; s <= N - 2; s += gridDim.x) {
         const int64_t K = (N - 1 - s + NBW - 1) >> LG;
         const int64_t Kprev = (N - s + NBW - 1) >> LG;      // K(s-1)
         uint32_t known = 0;
         for (int64_t k = 0; k < K; ++k) {
+            uint32_t need_head = 0;
             if (s > 0) {
-                const uint32_t need = (uint32_t)((k + 3 < Kprev) ? k + 3 : Kprev);
+                // everything but the corner of the block below: step (s-1, k+1) finished
+                const uint32_t need = (uint32_t)((k + 2 < Kprev) ? k + 2 : Kprev);
                 if (tid == 0) {
                     while (known < need) {
-                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(prog + s - 1) : "memory");
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(done + s - 1) : "memory");
                     }
                 }
                 __syncthreads();
+                if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);    // step (s-1, k+2) exists: its beta is our corner
             }
-            bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc);
+            bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc, head + s, head + s - 1, need_head);
             __threadfence();
             __syncthreads();
-            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(prog + s), "r"((uint32_t)(k + 1)) : "memory");
+            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
         }
     }
 }
@@ -472,7 +497,7 @@ __global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, doub
 }
 
 // host: prog == nullptr (or nbw = 128): all wavefronts t = 3s + k, in order, on one stream;
-// otherwise the persistent kernel (prog: N zeroed counters).  *launches = kernels launched.
+// otherwise the persistent kernel (prog: 2 N zeroed counters).  *launches = kernels launched.
 template <int NBW>
 cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_tau, double *d, double *e,
                                cudaStream_t st, int64_t *launches, uint32_t *prog = nullptr, int nsm = 0)

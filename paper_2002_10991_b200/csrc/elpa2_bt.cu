@@ -275,8 +275,8 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
     if (nbw <= 64 && N >= 2 && !wavefront_only) {
         cudaMemPool_t pool = scratch_pool(&err);
         if (!pool) return (int)err;
-        if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
-        if ((err = cudaMemsetAsync(prog, 0, (size_t)N * sizeof(uint32_t), st)) != cudaSuccess) return (int)err;
+        if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)2 * N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
+        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) return (int)err;
     }
     switch (nbw) {
     case 32: err = launch_bulge_chase<32>(N, ab, hh_v, hh_tau, d, e, st, &nl, prog, sm_count()); break;
