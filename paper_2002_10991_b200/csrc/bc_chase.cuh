@@ -6,10 +6,11 @@
 //   rows r0 = s+1+k nbw .. r1 = min(s+(k+1) nbw, N-1), eliminated column c = s (k = 0) or r0-nbw;
 //   (v, tau, beta) from B[r0..r1][c]; B <- H^T B H on the three blocks that can be non-zero:
 //   (i) B[r0..r1][c+1..r0-1], (ii) the diagonal block (symmetric rank-2 form), (iii) the block below.
-// Parallelism: step (s+1, k) touches what steps (s+1, k-1) and (s, k+2) wrote (the latter's head
-// element is the corner of the former's block (iii)), and steps with equal 3s + k touch disjoint
-// rectangles of the lower band.  So wavefront t = 3s + k runs as ONE launch with one CTA per step
-// (about N / (3 nbw) CTAs), and stream order provides the dependency between wavefronts.
+// Parallelism: step (s+1, k) touches what steps (s+1, k-1), (s, k+1) and (s, k+2) wrote, but it shares
+// only ONE element with (s, k+2): the latter's head element is the corner of the former's block (iii).
+// Two schedules: a persistent kernel (one CTA per SM walks sweeps c, c+grid, ..; per-sweep "done" and
+// "head" flags; dependency chain 2 steps per sweep) and, as the fallback for the real nbw = 128 step and
+// on request, one launch per wavefront t = 3s + k with stream order as the dependency.
 // The band lives in global memory (L2-resident: (2 nbw + 1) N doubles); a CTA keeps v and the
 // two work vectors of block (ii) in shared memory.  Every sum runs in the order SURVEY O3 / the oracle
 // states and every product and sum is rounded separately (__dmul_rn / __dadd_rn: no FMA contraction):
@@ -374,20 +375,14 @@ __device__ __forceinline__ zc zrecip(zc z)        // 1 / z
 }
 
 template <int NBW>
-__global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t t, int64_t s_hi, zc *__restrict__ ab,
-                                                             zc *__restrict__ hh_v, zc *__restrict__ hh_tau)
+__device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t s, const int64_t k, zc *__restrict__ ab,
+                                                 zc *__restrict__ hh_v, zc *__restrict__ hh_tau, zc *v, zc *p, zc *w2,
+                                                 zc *zsc, double *dsc, uint32_t *head_mine = nullptr,
+                                                 const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     constexpr int64_t ldab = 2 * NBW + 1;
-    __shared__ zc v[NBW], p[NBW], w2[NBW];
-    __shared__ zc s_tau, s_scal;
-    __shared__ double s_beta;
     const int tid = threadIdx.x, nt = blockDim.x;
-    const int64_t s = s_hi - blockIdx.x;
-    if (s < 0) return;
-    const int64_t k = t - 3 * s;
-    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
-    if (k < 0 || k >= K) return;
     const int64_t r0 = s + 1 + (k << LG);
     int64_t r1 = s + ((k + 1) << LG);
     if (r1 > N - 1) r1 = N - 1;
@@ -398,7 +393,10 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t 
     zc *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {
         for (int i = tid; i < NBW; i += nt) vout[i] = {(i == 0) ? 1.0 : 0.0, 0.0};
-        if (tid == 0) hh_tau[g] = {0.0, 0.0};
+        if (tid == 0) {
+            hh_tau[g] = {0.0, 0.0};
+            if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+        }
         return;
     }
     // --- Householder generator (R2, R7): beta real, tau = ((beta - Re a)/beta, -Im a/beta), v = x/(alpha - beta)
@@ -409,30 +407,33 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t 
         double ss = 0.0;
         for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dadd_rn(__dmul_rn(p[i].re, p[i].re), __dmul_rn(p[i].im, p[i].im)));
         if (ss == 0.0 && ai == 0.0) {
-            s_tau = {0.0, 0.0};
-            s_scal = {0.0, 0.0};
-            s_beta = ar;
+            zsc[0] = {0.0, 0.0};
+            zsc[1] = {0.0, 0.0};
+            dsc[0] = ar;
         } else {
             const double nrm = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(ar, ar), __dmul_rn(ai, ai)), ss));
             const double b = (ar >= 0.0) ? -nrm : nrm;
-            s_tau = {__ddiv_rn(__dsub_rn(b, ar), b), __ddiv_rn(-ai, b)};
-            s_scal = zrecip({__dsub_rn(ar, b), ai});
-            s_beta = b;
+            zsc[0] = {__ddiv_rn(__dsub_rn(b, ar), b), __ddiv_rn(-ai, b)};
+            zsc[1] = zrecip({__dsub_rn(ar, b), ai});
+            dsc[0] = b;
         }
     }
     __syncthreads();
-    const zc tau = s_tau, ctau = zconj(s_tau);
+    const zc tau = zsc[0], ctau = zconj(zsc[0]);
     const bool ident = (tau.re == 0.0 && tau.im == 0.0);
     for (int i = tid; i < NBW; i += nt) {
         zc vi = {0.0, 0.0};
         if (i == 0) vi = {1.0, 0.0};
-        else if (i < L && !ident) vi = zmul(p[i], s_scal);
+        else if (i < L && !ident) vi = zmul(p[i], zsc[1]);
         v[i] = vi;
         vout[i] = vi;
     }
     __syncthreads();
-    if (tid < L) BC_Z(r0 + tid, c) = {(tid == 0) ? s_beta : 0.0, 0.0};
-    if (tid == 0) hh_tau[g] = tau;
+    if (tid < L) BC_Z(r0 + tid, c) = {(tid == 0) ? dsc[0] : 0.0, 0.0};
+    if (tid == 0) {
+        hh_tau[g] = tau;
+        if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+    }
     if (ident) return;
     // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
     for (int64_t j = c + 1 + tid; j < r0; j += nt) {
@@ -470,11 +471,66 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t 
     int64_t r2 = r1 + NBW;
     if (r2 > N - 1) r2 = N - 1;
     for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
+        if (need_head && i == r2) {              // the corner is the head element of step (s-1, k+2): wait for its beta
+            uint32_t h;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+            } while (h < need_head);
+        }
         zc dot = {0.0, 0.0};
         for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
         for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
     }
 #undef BC_Z
+}
+
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t t, int64_t s_hi, zc *__restrict__ ab,
+                                                             zc *__restrict__ hh_v, zc *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    __shared__ zc v[NBW], p[NBW], w2[NBW], zsc[2];
+    __shared__ double dsc[1];
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc);
+}
+
+// persistent complex version: same flags and 2-step lag as bc_persistent_kernel, step on global memory
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_persistent_kernel_z(int64_t N, zc *__restrict__ ab, zc *__restrict__ hh_v,
+                                                              zc *__restrict__ hh_tau, uint32_t *__restrict__ prog)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    __shared__ zc v[NBW], p[NBW], w2[NBW], zsc[2];
+    __shared__ double dsc[1];
+    const int tid = threadIdx.x;
+    uint32_t *done = prog, *head = prog + N;
+    for (int64_t s = blockIdx.x; s <= N - 2; s += gridDim.x) {
+        const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+        const int64_t Kprev = (N - s + NBW - 1) >> LG;
+        uint32_t known = 0;
+        for (int64_t k = 0; k < K; ++k) {
+            uint32_t need_head = 0;
+            if (s > 0) {
+                const uint32_t need = (uint32_t)((k + 2 < Kprev) ? k + 2 : Kprev);
+                if (tid == 0) {
+                    while (known < need) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(done + s - 1) : "memory");
+                    }
+                }
+                __syncthreads();
+                if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
+            }
+            bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
+        }
+    }
 }
 
 template <int NBW>
@@ -565,11 +621,18 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
 // complex: the same wavefronts, global-memory step
 template <int NBW>
 cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double *d, double *e, cudaStream_t st,
-                                 int64_t *launches)
+                                 int64_t *launches, uint32_t *prog = nullptr, int nsm = 0)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     int64_t nl = 0;
-    if (N >= 2) {
+    if (prog && nsm > 0 && N >= 2) {
+        // one CTA per SM: resident by construction (the flag waits between sweeps rely on it)
+        const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
+        bc_persistent_kernel_z<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
+        ++nl;
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return e1;
+    } else if (N >= 2) {
         const int64_t Kmax = (N - 2 + NBW) >> LG;
         const int64_t tmax = (3 * (N - 2) > Kmax - 1) ? 3 * (N - 2) : Kmax - 1;
         for (int64_t t = 0; t <= tmax; ++t) {

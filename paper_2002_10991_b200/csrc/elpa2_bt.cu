@@ -306,10 +306,22 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, 
     cudaStream_t st = (cudaStream_t)stream;
     int64_t nl = 0;
     cudaError_t err;
+    static const bool wavefront_only = [] { const char *v = getenv("ELPA2_BC_WAVEFRONT"); return v && v[0] == '1'; }();
+    uint32_t *prog = nullptr;
+    if (N >= 2 && !wavefront_only) {
+        cudaMemPool_t pool = scratch_pool(&err);
+        if (!pool) return (int)err;
+        if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)2 * N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
+        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) return (int)err;
+    }
     switch (nbw) {
-    case 32: err = launch_bulge_chase_z<32>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
-    case 64: err = launch_bulge_chase_z<64>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
-    default: err = launch_bulge_chase_z<128>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl); break;
+    case 32: err = launch_bulge_chase_z<32>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl, prog, sm_count()); break;
+    case 64: err = launch_bulge_chase_z<64>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl, prog, sm_count()); break;
+    default: err = launch_bulge_chase_z<128>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl, prog, sm_count()); break;
+    }
+    if (prog) {
+        const cudaError_t e2 = cudaFreeAsync(prog, st);
+        if (err == cudaSuccess) err = e2;
     }
     if (err != cudaSuccess) return (int)err;
     g_last_launches = (int)(nl > 0x7fffffff ? 0x7fffffff : nl);
