@@ -9,8 +9,8 @@
 // Parallelism: step (s+1, k) touches what steps (s+1, k-1), (s, k+1) and (s, k+2) wrote, but it shares
 // only ONE element with (s, k+2): the latter's head element is the corner of the former's block (iii).
 // Two schedules: a persistent kernel (one CTA per SM walks sweeps c, c+grid, ..; per-sweep "done" and
-// "head" flags; dependency chain 2 steps per sweep) and, as the fallback for the real nbw = 128 step and
-// on request, one launch per wavefront t = 3s + k with stream order as the dependency.
+// "head" flags; dependency chain 2 steps per sweep) and, on request (ELPA2_BC_WAVEFRONT=1), one launch
+// per wavefront t = 3s + k with stream order as the dependency.
 // The band lives in global memory (L2-resident: (2 nbw + 1) N doubles); a CTA keeps v and the
 // two work vectors of block (ii) in shared memory.  Every sum runs in the order SURVEY O3 / the oracle
 // states and every product and sum is rounded separately (__dmul_rn / __dadd_rn: no FMA contraction):
@@ -23,19 +23,14 @@
 namespace elpa2bt {
 
 template <int NBW>
-__global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t, int64_t s_hi, double *__restrict__ ab,
-                                                           double *__restrict__ hh_v, double *__restrict__ hh_tau)
+__device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
+                                               double *__restrict__ hh_v, double *__restrict__ hh_tau, double *v, double *p,
+                                               double *w2, double *red, double *sc, uint32_t *head_mine = nullptr,
+                                               const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     constexpr int64_t ldab = 2 * NBW + 1;
-    __shared__ double v[NBW], p[NBW], w2[NBW], red[128];
-    __shared__ double s_tau, s_scal, s_beta;
     const int tid = threadIdx.x, nt = blockDim.x;
-    const int64_t s = s_hi - blockIdx.x;
-    if (s < 0) return;
-    const int64_t k = t - 3 * s;
-    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
-    if (k < 0 || k >= K) return;
     const int64_t r0 = s + 1 + (k << LG);
     int64_t r1 = s + ((k + 1) << LG);
     if (r1 > N - 1) r1 = N - 1;
@@ -46,7 +41,10 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
     double *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {                       // nothing to eliminate: identity slot (R3)
         for (int i = tid; i < NBW; i += nt) vout[i] = (i == 0) ? 1.0 : 0.0;
-        if (tid == 0) hh_tau[g] = 0.0;
+        if (tid == 0) {
+            hh_tau[g] = 0.0;
+            if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+        }
         return;
     }
     // --- Householder generator (R7): beta = -sign(alpha) ||x||, tau = (beta - alpha)/beta, v = x/(alpha - beta)
@@ -58,27 +56,30 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
 #pragma unroll 8
         for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dmul_rn(p[i], p[i]));
         if (ss == 0.0) {
-            s_tau = 0.0;
-            s_scal = 0.0;
-            s_beta = alpha;
+            sc[0] = 0.0;
+            sc[1] = 0.0;
+            sc[2] = alpha;
         } else {
             const double nrm = sqrt(__dadd_rn(__dmul_rn(alpha, alpha), ss));
             const double b = (alpha >= 0.0) ? -nrm : nrm;
-            s_tau = __ddiv_rn(__dsub_rn(b, alpha), b);
-            s_scal = __ddiv_rn(1.0, __dsub_rn(alpha, b));
-            s_beta = b;
+            sc[0] = __ddiv_rn(__dsub_rn(b, alpha), b);
+            sc[1] = __ddiv_rn(1.0, __dsub_rn(alpha, b));
+            sc[2] = b;
         }
     }
     __syncthreads();
-    const double tau = s_tau;
+    const double tau = sc[0];
     for (int i = tid; i < NBW; i += nt) {
-        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], s_scal) : 0.0);
+        const double vi = (i == 0) ? 1.0 : (i < L ? __dmul_rn(p[i], sc[1]) : 0.0);
         v[i] = vi;
         vout[i] = vi;
     }
     __syncthreads();
-    if (tid < L) BC_B(r0 + tid, c) = (tid == 0) ? s_beta : 0.0;
-    if (tid == 0) hh_tau[g] = tau;
+    if (tid < L) BC_B(r0 + tid, c) = (tid == 0) ? sc[2] : 0.0;
+    if (tid == 0) {
+        hh_tau[g] = tau;
+        if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+    }
     if (tau == 0.0) return;
     // --- (i) A <- H^T A on the rest of the bulge block: one thread per column
     for (int64_t j = c + 1 + tid; j < r0; j += nt) {
@@ -114,11 +115,66 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
     int64_t r2 = r1 + NBW;
     if (r2 > N - 1) r2 = N - 1;
     for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
+        if (need_head && i == r2) {              // the corner is the head element of step (s-1, k+2): wait for its beta
+            uint32_t h;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+            } while (h < need_head);
+        }
         double dot = 0.0;
         for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BC_B(i, r0 + l), v[l]));
         for (int l = 0; l < L; ++l) BC_B(i, r0 + l) = __dsub_rn(BC_B(i, r0 + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
     }
 #undef BC_B
+}
+
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t, int64_t s_hi, double *__restrict__ ab,
+                                                           double *__restrict__ hh_v, double *__restrict__ hh_tau)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    __shared__ double v[NBW], p[NBW], w2[NBW], red[128], sc[3];
+    const int64_t s = s_hi - blockIdx.x;
+    if (s < 0) return;
+    const int64_t k = t - 3 * s;
+    const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+    if (k < 0 || k >= K) return;
+    bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc);
+}
+
+// persistent version of the global-memory step (used for nbw = 128): flags and 2-step lag as in
+// bc_persistent_kernel below
+template <int NBW>
+__global__ void __launch_bounds__(128) bc_persistent_global_kernel(int64_t N, double *__restrict__ ab,
+                                                                   double *__restrict__ hh_v, double *__restrict__ hh_tau,
+                                                                   uint32_t *__restrict__ prog)
+{
+    constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    __shared__ double v[NBW], p[NBW], w2[NBW], red[128], sc[3];
+    const int tid = threadIdx.x;
+    uint32_t *done = prog, *head = prog + N;
+    for (int64_t s = blockIdx.x; s <= N - 2; s += gridDim.x) {
+        const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+        const int64_t Kprev = (N - s + NBW - 1) >> LG;
+        uint32_t known = 0;
+        for (int64_t k = 0; k < K; ++k) {
+            uint32_t need_head = 0;
+            if (s > 0) {
+                const uint32_t need = (uint32_t)((k + 2 < Kprev) ? k + 2 : Kprev);
+                if (tid == 0) {
+                    while (known < need) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(done + s - 1) : "memory");
+                    }
+                }
+                __syncthreads();
+                if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
+            }
+            bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc, head + s, head + s - 1, need_head);
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
+        }
+    }
 }
 
 // ---- the same step with its three blocks staged in shared memory (nbw <= 64) -------------------------
@@ -570,7 +626,13 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
             attr_done = true;
         }
     }
-    if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
+    if (NBW > 64 && prog && nsm > 0 && N >= 2) {
+        const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
+        bc_persistent_global_kernel<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
+        ++nl;
+        cudaError_t e1 = cudaGetLastError();
+        if (e1 != cudaSuccess) return e1;
+    } else if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
         auto pk = bc_persistent_kernel<(NBW <= 64 ? NBW : 64)>;
         static bool pattr_done = false;
         if (!pattr_done) {

@@ -268,11 +268,11 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
     cudaStream_t st = (cudaStream_t)stream;
     int64_t nl = 0;
     cudaError_t err;
-    // persistent kernel (nbw <= 64) unless ELPA2_BC_WAVEFRONT=1 asks for one launch per wavefront; its
+    // persistent kernel unless ELPA2_BC_WAVEFRONT=1 asks for one launch per wavefront; its
     // per-sweep progress counters come from the stream-ordered scratch pool
     static const bool wavefront_only = [] { const char *v = getenv("ELPA2_BC_WAVEFRONT"); return v && v[0] == '1'; }();
     uint32_t *prog = nullptr;
-    if (nbw <= 64 && N >= 2 && !wavefront_only) {
+    if (N >= 2 && !wavefront_only) {
         cudaMemPool_t pool = scratch_pool(&err);
         if (!pool) return (int)err;
         if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)2 * N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
@@ -281,7 +281,7 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
     switch (nbw) {
     case 32: err = launch_bulge_chase<32>(N, ab, hh_v, hh_tau, d, e, st, &nl, prog, sm_count()); break;
     case 64: err = launch_bulge_chase<64>(N, ab, hh_v, hh_tau, d, e, st, &nl, prog, sm_count()); break;
-    default: err = launch_bulge_chase<128>(N, ab, hh_v, hh_tau, d, e, st, &nl); break;
+    default: err = launch_bulge_chase<128>(N, ab, hh_v, hh_tau, d, e, st, &nl, prog, sm_count()); break;
     }
     if (prog) {
         const cudaError_t e2 = cudaFreeAsync(prog, st);

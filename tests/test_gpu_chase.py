@@ -54,6 +54,30 @@ def test_chase_matches_oracle(N, nbw, cplx):
     assert np.abs(t[:, 2:]).max(initial=0.0) <= 1e-12 * scale * max(N, 1)
 
 
+def test_wavefront_schedule_is_bit_identical():
+    """ELPA2_BC_WAVEFRONT=1 (one launch per wavefront 3s + k) in a fresh process: same bits as the oracle."""
+    import os
+    import subprocess
+    import sys
+
+    code = (
+        "import numpy as np, torch, oracle as orc\n"
+        "from paper_2002_10991_b200 import binding, synth_inputs as si\n"
+        "for cplx, N, nbw in ((False, 300, 64), (True, 200, 32), (False, 300, 128)):\n"
+        "    ab = si.band_matrix(N, nbw, 9, cplx); ab_o = ab.copy(order='F')\n"
+        "    hv_o, ht_o, d_o, e_o = orc.bulge_chase(ab_o, nbw)\n"
+        "    hv, ht, d, e = binding.bulge_chase(N, nbw, torch.from_numpy(np.ascontiguousarray(ab.T)).cuda())\n"
+        "    torch.cuda.synchronize()\n"
+        "    assert binding.last_launch_count() > 100\n"
+        "    assert np.array_equal(hv.cpu().numpy(), hv_o) and np.array_equal(ht.cpu().numpy(), ht_o)\n"
+        "    assert np.array_equal(d.cpu().numpy(), d_o) and np.array_equal(e.cpu().numpy(), e_o)\n"
+        "print('ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, ELPA2_BC_WAVEFRONT="1", PYTHONPATH=root + os.pathsep + os.path.join(root, "tests"))
+    out = subprocess.run([sys.executable, "-c", code], capture_output=True, text=True, timeout=300, cwd=root, env=env)
+    assert out.returncode == 0 and out.stdout.strip().endswith("ok"), out.stderr[-2000:]
+
+
 @pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("N,nbw", [(64, 32), (257, 64)])
 def test_chase_eigenvalues_and_end_to_end(N, nbw, cplx):
