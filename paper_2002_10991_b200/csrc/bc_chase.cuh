@@ -589,6 +589,208 @@ __global__ void __launch_bounds__(128) bc_persistent_kernel_z(int64_t N, zc *__r
     }
 }
 
+// ---- complex step with its blocks staged in shared memory (nbw <= 64) ----------------------------------
+// Two tiles: TA = block (i), nA columns x L rows (column stride NBW+1 elements); TB = blocks (ii)+(iii),
+// L columns x nR rows (column stride 2 NBW + 1): 198 KB at nbw = 64.  Arithmetic as bc_step_global_z.
+template <int NBW>
+__device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s, const int64_t k, zc *__restrict__ ab,
+                                               zc *__restrict__ hh_v, zc *__restrict__ hh_tau, zc *TA, zc *TB, zc *v, zc *p,
+                                               zc *w2, zc *zsc, double *dsc, uint32_t *head_mine,
+                                               const uint32_t *head_prev, const uint32_t need_head)
+{
+    constexpr int LG = (NBW == 32) ? 5 : 6;
+    constexpr int64_t ldab = 2 * NBW + 1;
+    constexpr int LDA = NBW + 1, LDB = 2 * NBW + 1;
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int64_t r0 = s + 1 + (k << LG);
+    int64_t r1 = s + ((k + 1) << LG);
+    if (r1 > N - 1) r1 = N - 1;
+    const int L = (int)(r1 - r0 + 1);
+    const int64_t c = (k == 0) ? s : r0 - NBW;
+    const int64_t g = hh_off(N, LG, s) + k;
+    zc *vout = hh_v + g * NBW;
+    if (k > 0 && L == 1) {
+        for (int i = tid; i < NBW; i += nt) vout[i] = {(i == 0) ? 1.0 : 0.0, 0.0};
+        if (tid == 0) {
+            hh_tau[g] = {0.0, 0.0};
+            asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+        }
+        return;
+    }
+    int64_t r2 = r1 + NBW;
+    if (r2 > N - 1) r2 = N - 1;
+    const int nA = (int)(r0 - c - 1), nR = (int)(r2 - r0 + 1);
+    // element (r0 + row, col j) of the band: ab[(r0 + row - j) + j * ldab]
+    const int Lp = (L + 31) & ~31, nRp = (nR + 31) & ~31;
+#pragma unroll 4
+    for (int e = tid; e < nA * Lp; e += nt) {
+        const int q = e / Lp, row = e - q * Lp;
+        if (row < L) {
+            const int64_t j = c + 1 + q;
+            cp_async16(smem_u32(&TA[q * LDA + row]), &ab[(r0 + row - j) + j * ldab], 16u);
+        }
+    }
+#pragma unroll 4
+    for (int e = tid; e < L * nRp; e += nt) {
+        const int q = e / nRp, row = e - q * nRp;
+        if (row >= q && row < nR) {
+            const int64_t j = r0 + q;
+            cp_async16(smem_u32(&TB[q * LDB + row]), &ab[(r0 + row - j) + j * ldab], 16u);
+        }
+    }
+    cp_async_commit();
+    if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];
+    cp_async_wait_all();
+    __syncthreads();
+    if (tid == 0) {
+        const double ar = p[0].re, ai = p[0].im;
+        double ss = 0.0;
+#pragma unroll 8
+        for (int i = 1; i < L; ++i) ss = __dadd_rn(ss, __dadd_rn(__dmul_rn(p[i].re, p[i].re), __dmul_rn(p[i].im, p[i].im)));
+        if (ss == 0.0 && ai == 0.0) {
+            zsc[0] = {0.0, 0.0};
+            zsc[1] = {0.0, 0.0};
+            dsc[0] = ar;
+        } else {
+            const double nrm = sqrt(__dadd_rn(__dadd_rn(__dmul_rn(ar, ar), __dmul_rn(ai, ai)), ss));
+            const double b = (ar >= 0.0) ? -nrm : nrm;
+            zsc[0] = {__ddiv_rn(__dsub_rn(b, ar), b), __ddiv_rn(-ai, b)};
+            zsc[1] = zrecip({__dsub_rn(ar, b), ai});
+            dsc[0] = b;
+        }
+    }
+    __syncthreads();
+    const zc tau = zsc[0], ctau = zconj(zsc[0]);
+    const bool ident = (tau.re == 0.0 && tau.im == 0.0);
+    for (int i = tid; i < NBW; i += nt) {
+        zc vi = {0.0, 0.0};
+        if (i == 0) vi = {1.0, 0.0};
+        else if (i < L && !ident) vi = zmul(p[i], zsc[1]);
+        v[i] = vi;
+        vout[i] = vi;
+    }
+    if (tid < L) ab[(r0 + tid - c) + c * ldab] = {(tid == 0) ? dsc[0] : 0.0, 0.0};
+    if (tid == 0) {
+        hh_tau[g] = tau;
+        asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
+    }
+    __syncthreads();
+    if (ident) return;
+#define ZA(rl, q) TA[(q) * LDA + (rl)]
+#define ZB(rl, q) TB[(q) * LDB + (rl)]
+    const int grp = tid >> 6, t64 = tid & 63;
+    if (grp == 0) {
+        // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
+        for (int q = t64; q < nA; q += 64) {
+            zc dot = {0.0, 0.0};
+#pragma unroll 4
+            for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), ZA(i, q)));
+#pragma unroll 4
+            for (int i = 0; i < L; ++i) ZA(i, q) = zsub(ZA(i, q), zmul(zmul(ctau, v[i]), dot));
+        }
+    } else if (grp == 1) {
+        // --- (iii) E <- E H = E - tau (E v) v^H
+        for (int rl = L + t64; rl < nR; rl += 64) {
+            if (need_head && rl == nR - 1) {
+                uint32_t h;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                } while (h < need_head);
+                const int64_t jc = r0 + L - 1;
+                const double2 cv = __ldcg(reinterpret_cast<const double2 *>(&ab[(r0 + rl - jc) + jc * ldab]));
+                ZB(rl, L - 1) = {cv.x, cv.y};
+            }
+            zc dot = {0.0, 0.0};
+#pragma unroll 4
+            for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(ZB(rl, l), v[l]));
+#pragma unroll 4
+            for (int l = 0; l < L; ++l) ZB(rl, l) = zsub(ZB(rl, l), zmul(zmul(tau, dot), zconj(v[l])));
+        }
+    } else if (grp == 2) {
+        // --- (ii) D(i, j) = ZB(i, j) (i >= j) or conj(ZB(j, i))
+        for (int j = t64; j < L; j += 64) {
+            zc dot = {0.0, 0.0};
+#pragma unroll 4
+            for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), (i >= j) ? ZB(i, j) : zconj(ZB(j, i))));
+            p[j] = dot;
+        }
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        for (int i = t64; i < L; i += 64) {
+            zc dot = {0.0, 0.0};
+#pragma unroll 4
+            for (int j = 0; j < L; ++j) {
+                const zc dij = (i >= j) ? ZB(i, j) : zconj(ZB(j, i));
+                const zc m = zsub(dij, zmul(zmul(ctau, v[i]), p[j]));
+                dot = zadd(dot, zmul(m, v[j]));
+            }
+            w2[i] = dot;
+        }
+        asm volatile("bar.sync 1, 64;" ::: "memory");
+        for (int j = t64; j < L; j += 64)
+            for (int i = j; i < L; ++i) {
+                const zc m = zsub(ZB(i, j), zmul(zmul(ctau, v[i]), p[j]));
+                zc r = zsub(m, zmul(zmul(tau, w2[i]), zconj(v[j])));
+                if (i == j) r.im = 0.0;
+                ZB(i, j) = r;
+            }
+    }
+    __syncthreads();
+#undef ZA
+#undef ZB
+#pragma unroll 4
+    for (int e = tid; e < nA * Lp; e += nt) {
+        const int q = e / Lp, row = e - q * Lp;
+        if (row < L) {
+            const int64_t j = c + 1 + q;
+            ab[(r0 + row - j) + j * ldab] = TA[q * LDA + row];
+        }
+    }
+#pragma unroll 4
+    for (int e = tid; e < L * nRp; e += nt) {
+        const int q = e / nRp, row = e - q * nRp;
+        if (row >= q && row < nR) {
+            const int64_t j = r0 + q;
+            ab[(r0 + row - j) + j * ldab] = TB[q * LDB + row];
+        }
+    }
+}
+
+template <int NBW>
+__global__ void __launch_bounds__(256) bc_persistent_smem_kernel_z(int64_t N, zc *__restrict__ ab, zc *__restrict__ hh_v,
+                                                                   zc *__restrict__ hh_tau, uint32_t *__restrict__ prog)
+{
+    constexpr int LG = (NBW == 32) ? 5 : 6;
+    extern __shared__ __align__(16) unsigned char zsm[];
+    zc *TA = reinterpret_cast<zc *>(zsm);
+    zc *TB = TA + (NBW - 1) * (NBW + 1);
+    __shared__ zc v[NBW], p[NBW], w2[NBW], zsc[2];
+    __shared__ double dsc[1];
+    const int tid = threadIdx.x;
+    uint32_t *done = prog, *head = prog + N;
+    for (int64_t s = blockIdx.x; s <= N - 2; s += gridDim.x) {
+        const int64_t K = (N - 1 - s + NBW - 1) >> LG;
+        const int64_t Kprev = (N - s + NBW - 1) >> LG;
+        uint32_t known = 0;
+        for (int64_t k = 0; k < K; ++k) {
+            uint32_t need_head = 0;
+            if (s > 0) {
+                const uint32_t need = (uint32_t)((k + 2 < Kprev) ? k + 2 : Kprev);
+                if (tid == 0) {
+                    while (known < need) {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(known) : "l"(done + s - 1) : "memory");
+                    }
+                }
+                __syncthreads();
+                if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
+            }
+            bc_step_smem_z<NBW>(N, s, k, ab, hh_v, hh_tau, TA, TB, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
+            __threadfence();
+            __syncthreads();
+            if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
+        }
+    }
+}
+
 template <int NBW>
 __global__ void bc_extract_kernel_z(int64_t N, const zc *__restrict__ ab, double *__restrict__ d, double *__restrict__ e)
 {
@@ -690,7 +892,19 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
     if (prog && nsm > 0 && N >= 2) {
         // one CTA per SM: resident by construction (the flag waits between sweeps rely on it)
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        bc_persistent_kernel_z<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
+        if (NBW <= 64) {
+            constexpr int NB = (NBW <= 64) ? NBW : 64;
+            constexpr int zbytes = ((NB - 1) * (NB + 1) + NB * (2 * NB + 1)) * 16;
+            auto zk = bc_persistent_smem_kernel_z<NB>;
+            static bool zattr = false;
+            if (!zattr) {
+                cudaError_t e0 = cudaFuncSetAttribute(zk, cudaFuncAttributeMaxDynamicSharedMemorySize, zbytes);
+                if (e0 != cudaSuccess) return e0;
+                zattr = true;
+            }
+            zk<<<(unsigned)grid, 256, zbytes, st>>>(N, ab, hh_v, hh_tau, prog);
+        } else
+            bc_persistent_kernel_z<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
         ++nl;
         cudaError_t e1 = cudaGetLastError();
         if (e1 != cudaSuccess) return e1;
