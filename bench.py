@@ -188,6 +188,16 @@ def run_reference(args, rank: int) -> None:
     }), flush=True)
 
 
+def chase_kernel_name(cplx: bool, nbw: int) -> str:
+    """The kernel elpa2_bulge_chase_{d,z} launches (csrc/bc_chase.cuh), for the JSON line."""
+    if os.environ.get("ELPA2_BC_WAVEFRONT", "")[:1] == "1":
+        return ("bc_wavefront_kernel_z" if cplx else
+                ("bc_wavefront_smem_kernel" if nbw <= 64 else "bc_wavefront_kernel")) + " (one launch per wavefront)"
+    if cplx:
+        return "bc_persistent_smem_kernel_z" if nbw <= 64 else "bc_persistent_kernel_z"
+    return "bc_persistent_kernel" if nbw <= 64 else "bc_persistent_global_kernel"
+
+
 def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
     """--chase: SURVEY.md 8(f) NEXT-1, first version.  One step = one band -> tridiagonal reduction of the
     config's seeded band matrix on the device (about 3N wavefront launches); model work 6 N^2 nbw flops
@@ -241,7 +251,7 @@ def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
                        "parallelism": "replicas only", "l2": "band matrix restored from host before every step"},
             "roofline": {"bound": "alu", "achieved": achieved, "peak": dfma_tf, "unit": "TFLOP/s", "frac": achieved / dfma_tf,
                          "peak_source": "DFMA probe of this run; first version: launch- and latency-bound",
-                         "kernel": "bc_wavefront_kernel_z" if cplx else "bc_wavefront_smem_kernel", "kernel_ms": ms,
+                         "kernel": chase_kernel_name(cplx, nbw), "kernel_ms": ms,
                          "traffic": None},
             "clocks": clocks.summary(), "e2e": None, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"relative_trace_error": tr_err},
