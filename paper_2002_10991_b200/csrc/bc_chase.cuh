@@ -222,18 +222,17 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
             hi = nR;
         }
     };
-    // --- stage in: flat loop over (column, row) so that many independent loads are in flight; lanes run
-    //     along the contiguous band segment of a column
-    const int nRp = (nR + 31) & ~31;
-#pragma unroll 4
-    for (int e = tid; e < ncol * nRp; e += nt) {
-        const int q = e / nRp, row = e - q * nRp;
+    // --- stage in: a warp per column, lanes along the column's contiguous band segment; cp.async keeps
+    //     every copy in flight at once (no index arithmetic worth mentioning: a flat (column, row) loop
+    //     spent more time on its divisions than on the copies)
+    const int warp = tid >> 5, lane = tid & 31, nwarp = nt >> 5;
+    for (int q = warp; q < ncol; q += nwarp) {
         int lo, hi;
         seg(q, lo, hi);
-        if (row >= lo && row < hi) {
-            const int64_t j = c + 1 + q;
-            cp_async8(smem_u32(&S[q * LDS + row]), &ab[(r0 + row - j) + j * ldab], 8u);   // all copies in flight at once
-        }
+        const int64_t j = c + 1 + q;
+        const double *src = ab + (r0 - j) + j * ldab;          // element (r0 + row, j) at src[row]
+        double *dst = S + q * LDS;
+        for (int row = lo + lane; row < hi; row += 32) cp_async8(smem_u32(dst + row), src + row, 8u);
     }
     cp_async_commit();
     if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];       // x = B[r0..r1][c]
@@ -334,15 +333,13 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
     __syncthreads();
 #undef BS
     // --- stage out
-#pragma unroll 4
-    for (int e = tid; e < ncol * nRp; e += nt) {
-        const int q = e / nRp, row = e - q * nRp;
+    for (int q = warp; q < ncol; q += nwarp) {
         int lo, hi;
         seg(q, lo, hi);
-        if (row >= lo && row < hi) {
-            const int64_t j = c + 1 + q;
-            ab[(r0 + row - j) + j * ldab] = S[q * LDS + row];
-        }
+        const int64_t j = c + 1 + q;
+        double *dst = ab + (r0 - j) + j * ldab;
+        const double *src = S + q * LDS;
+        for (int row = lo + lane; row < hi; row += 32) dst[row] = src[row];
     }
 }
 
@@ -621,22 +618,13 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
     if (r2 > N - 1) r2 = N - 1;
     const int nA = (int)(r0 - c - 1), nR = (int)(r2 - r0 + 1);
     // element (r0 + row, col j) of the band: ab[(r0 + row - j) + j * ldab]
-    const int Lp = (L + 31) & ~31, nRp = (nR + 31) & ~31;
-#pragma unroll 4
-    for (int e = tid; e < nA * Lp; e += nt) {
-        const int q = e / Lp, row = e - q * Lp;
-        if (row < L) {
-            const int64_t j = c + 1 + q;
-            cp_async16(smem_u32(&TA[q * LDA + row]), &ab[(r0 + row - j) + j * ldab], 16u);
-        }
-    }
-#pragma unroll 4
-    for (int e = tid; e < L * nRp; e += nt) {
-        const int q = e / nRp, row = e - q * nRp;
-        if (row >= q && row < nR) {
-            const int64_t j = r0 + q;
-            cp_async16(smem_u32(&TB[q * LDB + row]), &ab[(r0 + row - j) + j * ldab], 16u);
-        }
+    const int warp = tid >> 5, lane = tid & 31, nwarp = nt >> 5;
+    for (int q = warp; q < nA + L; q += nwarp) {          // a warp per column, lanes along its band segment
+        const int64_t j = c + 1 + q;
+        const zc *src = ab + (r0 - j) + j * ldab;
+        zc *dst = (q < nA) ? TA + q * LDA : TB + (q - nA) * LDB;
+        const int lo = (q < nA) ? 0 : q - nA, hi = (q < nA) ? L : nR;
+        for (int row = lo + lane; row < hi; row += 32) cp_async16(smem_u32(dst + row), src + row, 16u);
     }
     cp_async_commit();
     if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];
@@ -737,21 +725,12 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
     __syncthreads();
 #undef ZA
 #undef ZB
-#pragma unroll 4
-    for (int e = tid; e < nA * Lp; e += nt) {
-        const int q = e / Lp, row = e - q * Lp;
-        if (row < L) {
-            const int64_t j = c + 1 + q;
-            ab[(r0 + row - j) + j * ldab] = TA[q * LDA + row];
-        }
-    }
-#pragma unroll 4
-    for (int e = tid; e < L * nRp; e += nt) {
-        const int q = e / nRp, row = e - q * nRp;
-        if (row >= q && row < nR) {
-            const int64_t j = r0 + q;
-            ab[(r0 + row - j) + j * ldab] = TB[q * LDB + row];
-        }
+    for (int q = warp; q < nA + L; q += nwarp) {
+        const int64_t j = c + 1 + q;
+        zc *dst = ab + (r0 - j) + j * ldab;
+        const zc *src = (q < nA) ? TA + q * LDA : TB + (q - nA) * LDB;
+        const int lo = (q < nA) ? 0 : q - nA, hi = (q < nA) ? L : nR;
+        for (int row = lo + lane; row < hi; row += 32) dst[row] = src[row];
     }
 }
 
