@@ -789,6 +789,17 @@ __global__ void bc_extract_kernel(int64_t N, const double *__restrict__ ab, doub
     if (i + 1 < N) e[i] = ab[1 + i * ldab];
 }
 
+// The persistent kernels wait on flags written by other CTAs of the same grid, so every CTA of the grid
+// must be resident at once: a cooperative launch (no grid.sync is used) makes the driver guarantee that,
+// or fail, instead of leaving it to how busy the device happens to be.
+template <class K, class T>
+cudaError_t bc_launch_persistent(K kern, int64_t grid, int threads, size_t smem, cudaStream_t st, int64_t N, T *ab, T *hh_v,
+                                 T *hh_tau, uint32_t *prog)
+{
+    void *args[] = {(void *)&N, (void *)&ab, (void *)&hh_v, (void *)&hh_tau, (void *)&prog};
+    return cudaLaunchCooperativeKernel((const void *)kern, dim3((unsigned)grid), dim3((unsigned)threads), args, smem, st);
+}
+
 // host: prog == nullptr (or nbw = 128): all wavefronts t = 3s + k, in order, on one stream;
 // otherwise the persistent kernel (prog: 2 N zeroed counters).  *launches = kernels launched.
 template <int NBW>
@@ -809,9 +820,8 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     }
     if (NBW > 64 && prog && nsm > 0 && N >= 2) {
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        bc_persistent_global_kernel<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
+        cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 128, 0, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
-        cudaError_t e1 = cudaGetLastError();
         if (e1 != cudaSuccess) return e1;
     } else if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
         auto pk = bc_persistent_kernel<(NBW <= 64 ? NBW : 64)>;
@@ -824,9 +834,8 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
         // one CTA per SM (its tile takes more than half of an SM's shared memory): all CTAs are resident,
         // which the flag waits between sweeps rely on
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        pk<<<(unsigned)grid, 256, smem_bytes, st>>>(N, ab, hh_v, hh_tau, prog);
+        cudaError_t e1 = bc_launch_persistent(pk, grid, 256, smem_bytes, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
-        cudaError_t e1 = cudaGetLastError();
         if (e1 != cudaSuccess) return e1;
     } else if (N >= 2) {
         const int64_t Kmax = (N - 2 + NBW) >> LG;                  // K(0)
@@ -871,6 +880,7 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
     if (prog && nsm > 0 && N >= 2) {
         // one CTA per SM: resident by construction (the flag waits between sweeps rely on it)
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
+        cudaError_t e1 = cudaSuccess;
         if (NBW <= 64) {
             constexpr int NB = (NBW <= 64) ? NBW : 64;
             constexpr int zbytes = ((NB - 1) * (NB + 1) + NB * (2 * NB + 1)) * 16;
@@ -881,11 +891,10 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
                 if (e0 != cudaSuccess) return e0;
                 zattr = true;
             }
-            zk<<<(unsigned)grid, 256, zbytes, st>>>(N, ab, hh_v, hh_tau, prog);
+            e1 = bc_launch_persistent(zk, grid, 256, zbytes, st, N, ab, hh_v, hh_tau, prog);
         } else
-            bc_persistent_kernel_z<NBW><<<(unsigned)grid, 128, 0, st>>>(N, ab, hh_v, hh_tau, prog);
+            e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 128, 0, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
-        cudaError_t e1 = cudaGetLastError();
         if (e1 != cudaSuccess) return e1;
     } else if (N >= 2) {
         const int64_t Kmax = (N - 2 + NBW) >> LG;
