@@ -81,49 +81,63 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
         if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
     if (tau == 0.0) return;
-    // --- (i) A <- H^T A on the rest of the bulge block: one thread per column
-    for (int64_t j = c + 1 + tid; j < r0; j += nt) {
-        double dot = 0.0;
-        for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BC_B(r0 + i, j)));
-        for (int i = 0; i < L; ++i) BC_B(r0 + i, j) = __dsub_rn(BC_B(r0 + i, j), __dmul_rn(__dmul_rn(tau, v[i]), dot));
-    }
-    // --- (ii) D <- H^T D H: p = D v;  M = D - tau v p^T;  w2 = M v;  D' = M - tau w2 v^T (lower part)
-    __syncthreads();                              // p held x until here
-    for (int j = tid; j < L; j += nt) {
-        double dot = 0.0;
-        for (int i = 0; i < L; ++i)
-            dot = __dadd_rn(dot, __dmul_rn(v[i], (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i)));
-        red[j] = dot;
-    }
-    __syncthreads();
-    for (int i = tid; i < L; i += nt) {
-        double dot = 0.0;
-        for (int j = 0; j < L; ++j) {
-            const double dij = (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i);
-            const double m = __dsub_rn(dij, __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
-            dot = __dadd_rn(dot, __dmul_rn(m, v[j]));
+    // 384 threads (persistent kernel): three groups of 128 run (i), (iii), (ii) side by side; see bc_step_global_z
+    const bool par = nt >= 384;
+    const int grp = par ? (tid >> 7) : 0, t0 = par ? (tid & 127) : tid, st_ = par ? 128 : nt;
+    auto sync_ii = [&]() {
+        if (par)
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        else
+            __syncthreads();
+    };
+    if (!par || grp == 0) {
+        // --- (i) A <- H^T A on the rest of the bulge block: one thread per column
+        for (int64_t j = c + 1 + t0; j < r0; j += st_) {
+            double dot = 0.0;
+            for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BC_B(r0 + i, j)));
+            for (int i = 0; i < L; ++i) BC_B(r0 + i, j) = __dsub_rn(BC_B(r0 + i, j), __dmul_rn(__dmul_rn(tau, v[i]), dot));
         }
-        w2[i] = dot;
     }
-    __syncthreads();
-    for (int j = tid; j < L; j += nt)
-        for (int i = j; i < L; ++i) {
-            const double m = __dsub_rn(BC_B(r0 + i, r0 + j), __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
-            BC_B(r0 + i, r0 + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
+    if (!par || grp == 2) {
+        // --- (ii) D <- H^T D H: red = D v;  M = D - tau v red^T;  w2 = M v;  D' = M - tau w2 v^T (lower part)
+        for (int j = t0; j < L; j += st_) {
+            double dot = 0.0;
+            for (int i = 0; i < L; ++i)
+                dot = __dadd_rn(dot, __dmul_rn(v[i], (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i)));
+            red[j] = dot;
         }
-    // --- (iii) E <- E H on the block below: one thread per row; creates the next bulge
-    int64_t r2 = r1 + NBW;
-    if (r2 > N - 1) r2 = N - 1;
-    for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
-        if (need_head && i == r2) {              // the corner is the head element of step (s-1, k+2): wait for its beta
-            uint32_t h;
-            do {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
-            } while (h < need_head);
+        sync_ii();
+        for (int i = t0; i < L; i += st_) {
+            double dot = 0.0;
+            for (int j = 0; j < L; ++j) {
+                const double dij = (i >= j) ? BC_B(r0 + i, r0 + j) : BC_B(r0 + j, r0 + i);
+                const double m = __dsub_rn(dij, __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+                dot = __dadd_rn(dot, __dmul_rn(m, v[j]));
+            }
+            w2[i] = dot;
         }
-        double dot = 0.0;
-        for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BC_B(i, r0 + l), v[l]));
-        for (int l = 0; l < L; ++l) BC_B(i, r0 + l) = __dsub_rn(BC_B(i, r0 + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
+        sync_ii();
+        for (int j = t0; j < L; j += st_)
+            for (int i = j; i < L; ++i) {
+                const double m = __dsub_rn(BC_B(r0 + i, r0 + j), __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+                BC_B(r0 + i, r0 + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
+            }
+    }
+    if (!par || grp == 1) {
+        // --- (iii) E <- E H on the block below: one thread per row; creates the next bulge
+        int64_t r2 = r1 + NBW;
+        if (r2 > N - 1) r2 = N - 1;
+        for (int64_t i = r1 + 1 + t0; i <= r2; i += st_) {
+            if (need_head && i == r2) {          // the corner is the head element of step (s-1, k+2): wait for its beta
+                uint32_t h;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                } while (h < need_head);
+            }
+            double dot = 0.0;
+            for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BC_B(i, r0 + l), v[l]));
+            for (int l = 0; l < L; ++l) BC_B(i, r0 + l) = __dsub_rn(BC_B(i, r0 + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
+        }
     }
 #undef BC_B
 }
@@ -145,7 +159,7 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
 // persistent version of the global-memory step (used for nbw = 128): flags and 2-step lag as in
 // bc_persistent_kernel below
 template <int NBW>
-__global__ void __launch_bounds__(128) bc_persistent_global_kernel(int64_t N, double *__restrict__ ab,
+__global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, double *__restrict__ ab,
                                                                    double *__restrict__ hh_v, double *__restrict__ hh_tau,
                                                                    uint32_t *__restrict__ prog)
 {
@@ -488,51 +502,67 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
         if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
     if (ident) return;
-    // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
-    for (int64_t j = c + 1 + tid; j < r0; j += nt) {
-        zc dot = {0.0, 0.0};
-        for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), BC_Z(r0 + i, j)));
-        for (int i = 0; i < L; ++i) BC_Z(r0 + i, j) = zsub(BC_Z(r0 + i, j), zmul(zmul(ctau, v[i]), dot));
-    }
-    // --- (ii) D <- H^H D H: p = v^H D;  M = D - conj(tau) v p;  w2 = M v;  D' = M - tau w2 v^H (lower part)
-    __syncthreads();
-    for (int j = tid; j < L; j += nt) {
-        zc dot = {0.0, 0.0};
-        for (int i = 0; i < L; ++i)
-            dot = zadd(dot, zmul(zconj(v[i]), (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i))));
-        p[j] = dot;
-    }
-    __syncthreads();
-    for (int i = tid; i < L; i += nt) {
-        zc dot = {0.0, 0.0};
-        for (int j = 0; j < L; ++j) {
-            const zc dij = (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i));
-            const zc m = zsub(dij, zmul(zmul(ctau, v[i]), p[j]));
-            dot = zadd(dot, zmul(m, v[j]));
+    // With 384 threads (persistent kernel) three groups of 128 run the disjoint blocks (i), (iii), (ii) side
+    // by side ((ii) synchronises on a named barrier of its own); with fewer threads they run one after
+    // the other.  Same arithmetic either way.
+    const bool par = nt >= 384;
+    const int grp = par ? (tid >> 7) : 0, t0 = par ? (tid & 127) : tid, st_ = par ? 128 : nt;
+    auto sync_ii = [&]() {
+        if (par)
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+        else
+            __syncthreads();
+    };
+    if (!par || grp == 0) {
+        // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
+        for (int64_t j = c + 1 + t0; j < r0; j += st_) {
+            zc dot = {0.0, 0.0};
+            for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), BC_Z(r0 + i, j)));
+            for (int i = 0; i < L; ++i) BC_Z(r0 + i, j) = zsub(BC_Z(r0 + i, j), zmul(zmul(ctau, v[i]), dot));
         }
-        w2[i] = dot;
     }
-    __syncthreads();
-    for (int j = tid; j < L; j += nt)
-        for (int i = j; i < L; ++i) {
-            const zc m = zsub(BC_Z(r0 + i, r0 + j), zmul(zmul(ctau, v[i]), p[j]));
-            zc r = zsub(m, zmul(zmul(tau, w2[i]), zconj(v[j])));
-            if (i == j) r.im = 0.0;              // a Hermitian diagonal is real
-            BC_Z(r0 + i, r0 + j) = r;
+    if (!par || grp == 2) {
+        // --- (ii) D <- H^H D H: p = v^H D;  M = D - conj(tau) v p;  w2 = M v;  D' = M - tau w2 v^H (lower part)
+        for (int j = t0; j < L; j += st_) {
+            zc dot = {0.0, 0.0};
+            for (int i = 0; i < L; ++i)
+                dot = zadd(dot, zmul(zconj(v[i]), (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i))));
+            p[j] = dot;
         }
-    // --- (iii) E <- E H = E - tau (E v) v^H
-    int64_t r2 = r1 + NBW;
-    if (r2 > N - 1) r2 = N - 1;
-    for (int64_t i = r1 + 1 + tid; i <= r2; i += nt) {
-        if (need_head && i == r2) {              // the corner is the head element of step (s-1, k+2): wait for its beta
-            uint32_t h;
-            do {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
-            } while (h < need_head);
+        sync_ii();
+        for (int i = t0; i < L; i += st_) {
+            zc dot = {0.0, 0.0};
+            for (int j = 0; j < L; ++j) {
+                const zc dij = (i >= j) ? BC_Z(r0 + i, r0 + j) : zconj(BC_Z(r0 + j, r0 + i));
+                const zc m = zsub(dij, zmul(zmul(ctau, v[i]), p[j]));
+                dot = zadd(dot, zmul(m, v[j]));
+            }
+            w2[i] = dot;
         }
-        zc dot = {0.0, 0.0};
-        for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
-        for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
+        sync_ii();
+        for (int j = t0; j < L; j += st_)
+            for (int i = j; i < L; ++i) {
+                const zc m = zsub(BC_Z(r0 + i, r0 + j), zmul(zmul(ctau, v[i]), p[j]));
+                zc r = zsub(m, zmul(zmul(tau, w2[i]), zconj(v[j])));
+                if (i == j) r.im = 0.0;              // a Hermitian diagonal is real
+                BC_Z(r0 + i, r0 + j) = r;
+            }
+    }
+    if (!par || grp == 1) {
+        // --- (iii) E <- E H = E - tau (E v) v^H
+        int64_t r2 = r1 + NBW;
+        if (r2 > N - 1) r2 = N - 1;
+        for (int64_t i = r1 + 1 + t0; i <= r2; i += st_) {
+            if (need_head && i == r2) {          // the corner is the head element of step (s-1, k+2): wait for its beta
+                uint32_t h;
+                do {
+                    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                } while (h < need_head);
+            }
+            zc dot = {0.0, 0.0};
+            for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
+            for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
+        }
     }
 #undef BC_Z
 }
@@ -554,7 +584,7 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t 
 
 // persistent complex version: same flags and 2-step lag as bc_persistent_kernel, step on global memory
 template <int NBW>
-__global__ void __launch_bounds__(128) bc_persistent_kernel_z(int64_t N, zc *__restrict__ ab, zc *__restrict__ hh_v,
+__global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__restrict__ ab, zc *__restrict__ hh_v,
                                                               zc *__restrict__ hh_tau, uint32_t *__restrict__ prog)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
@@ -820,7 +850,7 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     }
     if (NBW > 64 && prog && nsm > 0 && N >= 2) {
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 128, 0, st, N, ab, hh_v, hh_tau, prog);
+        cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 384, 0, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
         if (e1 != cudaSuccess) return e1;
     } else if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
@@ -893,7 +923,7 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
             }
             e1 = bc_launch_persistent(zk, grid, 256, zbytes, st, N, ab, hh_v, hh_tau, prog);
         } else
-            e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 128, 0, st, N, ab, hh_v, hh_tau, prog);
+            e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 384, 0, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
         if (e1 != cudaSuccess) return e1;
     } else if (N >= 2) {
