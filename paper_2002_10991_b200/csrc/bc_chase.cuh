@@ -184,7 +184,8 @@ __global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, do
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
             bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc, head + s, head + s - 1, need_head);
-            __threadfence();
+            // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
+            // barriers are built from): one fence, not one per thread
             __syncthreads();
             if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
         }
@@ -409,7 +410,8 @@ __global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *_
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);    // step (s-1, k+2) exists: its beta is our corner
             }
             bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc, head + s, head + s - 1, need_head);
-            __threadfence();
+            // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
+            // barriers are built from): one fence, not one per thread
             __syncthreads();
             if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
         }
@@ -609,7 +611,8 @@ __global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__r
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
             bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
-            __threadfence();
+            // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
+            // barriers are built from): one fence, not one per thread
             __syncthreads();
             if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
         }
@@ -793,7 +796,8 @@ __global__ void __launch_bounds__(256) bc_persistent_smem_kernel_z(int64_t N, zc
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
             bc_step_smem_z<NBW>(N, s, k, ab, hh_v, hh_tau, TA, TB, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
-            __threadfence();
+            // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
+            // barriers are built from): one fence, not one per thread
             __syncthreads();
             if (tid == 0) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(done + s), "r"((uint32_t)(k + 1)) : "memory");
         }
