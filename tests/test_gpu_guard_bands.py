@@ -87,3 +87,25 @@ def test_bulge_chase_stays_inside_its_buffers(N, nbw, cplx):
     assert np.array_equal(dd.cpu().numpy(), d_o) and np.array_equal(de.cpu().numpy()[:N - 1], e_o)
     assert _guards_ok(wab, N * (2 * nbw + 1)) and _guards_ok(wv, G * nbw) and _guards_ok(wt, G)
     assert _guards_ok(wd, N) and _guards_ok(we, max(N - 1, 1))
+
+
+def test_real_q_that_is_only_8_byte_aligned():
+    """q starting one double past a 16-byte boundary: the kernel must take its 8-byte access path."""
+    import torch
+
+    from paper_2002_10991_b200 import binding
+
+    N, nbw, nev = 2 * 64 + 10, 64, 77
+    ab = si.band_matrix(N, nbw, 4, False)
+    hv, ht, _, _ = orc.bulge_chase(ab, nbw)
+    x = np.asfortranarray(np.random.default_rng(2).standard_normal((N, nev)))
+    want = oracle_apply(N, nbw, hv, ht, x)
+    whole = torch.full((N * nev + 2 * GUARD + 1,), SENT, dtype=torch.float64, device="cuda")
+    q_cm = whole[GUARD + 1:GUARD + 1 + N * nev].view(nev, N)
+    assert q_cm.data_ptr() % 16 == 8
+    q_cm.copy_(torch.from_numpy(np.ascontiguousarray(x.T)).cuda())
+    binding.trans_ev_tridi_to_band(N, nbw, torch.from_numpy(hv).cuda(), torch.from_numpy(ht).cuda(), q_cm.t())
+    torch.cuda.synchronize()
+    assert np.abs(q_cm.t().cpu().numpy() - want).max() <= 1e-11 * np.abs(x).max()
+    s_ = torch.full((1,), SENT, dtype=torch.float64, device="cuda")
+    assert bool((whole[:GUARD + 1] == s_).all().item()) and bool((whole[GUARD + 1 + N * nev:] == s_).all().item())
