@@ -155,6 +155,8 @@ def test_two_chains_per_pass_variant(nbw):
     _check(9 * nbw + 3, nbw, 148 * 8 * 2 + 21, False, variant=3)     # 2-3 slabs per CTA
     _check(8 * nbw, nbw, 5000, False, variant=3)
     _check(3 * nbw + 5, nbw, 100, False, variant=3)                  # too few chains: falls back to P = 1
+    if nbw == 32:
+        _check(9 * nbw + 3, nbw, 148 * 16 * 8 + 100, False, variant=3)  # more than one wave of CTAs, 4-slab warps
 
 
 def test_degenerate_no_work():
