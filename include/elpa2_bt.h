@@ -112,6 +112,11 @@ int elpa2_bt_set_variant(int variant);
  * of scratch }.  All zero when there is no work.  Returns 0 or -i for a bad i-th argument. */
 int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int64_t out[6]);
 
+/* Gives back what the library caches: the device buffers of the host-buffer entry point and the unused
+ * memory of the scratch pool (blocks still in use by enqueued calls stay).  Synchronises the device
+ * (cudaFree).  Returns 0 or a cudaError_t.  Without a device and with nothing cached: 0. */
+int elpa2_bt_release_scratch(void);
+
 const char *elpa2_bt_version(void);
 
 /* Measurement aid (synchronous; allocates and frees a small device buffer): sustained FP64 ALU

@@ -21,7 +21,7 @@ EXPORTS = (
     "elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z",
     "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
-    "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan",
+    "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
 )
 
 
@@ -54,6 +54,8 @@ def lib() -> ctypes.CDLL:
         for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
             getattr(L, nm).argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
             getattr(L, nm).restype = i32
+        L.elpa2_bt_release_scratch.argtypes = []
+        L.elpa2_bt_release_scratch.restype = i32
         L.elpa2_bt_plan.argtypes = [i32, i64, i32, i64, i32, ctypes.POINTER(i64)]
         L.elpa2_bt_plan.restype = i32
         L.elpa2_hh_count.argtypes = [i64, i32]
@@ -115,6 +117,13 @@ def plan(cplx: bool, N: int, nbw: int, nev: int, n_sm: int = 148) -> dict:
         raise Elpa2BtError(rc)
     keys = ("grid", "warps_per_cta", "P", "slabs", "slabs_per_cta_max", "scratch_bytes")
     return dict(zip(keys, (int(x) for x in out)))
+
+
+def release_scratch() -> None:
+    """Free the library's cached device memory (host-entry buffers, unused scratch-pool blocks)."""
+    rc = lib().elpa2_bt_release_scratch()
+    if rc != 0:
+        raise Elpa2BtError(rc)
 
 
 def version() -> str:

@@ -84,10 +84,13 @@ cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const doubl
 // stream-ordered scratch for the -T factors of the WY kernel: a private memory pool that keeps
 // what it has allocated (release threshold = max), so that in steady state a call allocates
 // nothing new and never synchronises the host
+cudaMemPool_t g_pool = nullptr;     // written under g_pool_mu
+int g_pool_dev = -1;
+
 cudaMemPool_t scratch_pool(cudaError_t *err)
 {
-    static cudaMemPool_t pool = nullptr;
-    static int pool_dev = -1;
+    cudaMemPool_t &pool = g_pool;
+    int &pool_dev = g_pool_dev;
     int dev = 0;
     *err = cudaGetDevice(&dev);
     if (*err != cudaSuccess) return nullptr;
@@ -373,6 +376,28 @@ int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int
     out[4] = pl.per_cta;
     out[5] = (int64_t)scratch;
     return 0;
+}
+
+int elpa2_bt_release_scratch(void)
+{
+    cudaError_t first = cudaSuccess;
+    {
+        std::lock_guard<std::mutex> lock(g_mu);
+        for (Scratch *s : {&g_sv, &g_st, &g_sq}) {
+            if (s->p) {
+                const cudaError_t e = cudaFree(s->p);
+                if (first == cudaSuccess) first = e;
+            }
+            s->p = nullptr;
+            s->cap = 0;
+        }
+    }
+    std::lock_guard<std::mutex> lock(g_pool_mu);
+    if (g_pool) {
+        const cudaError_t e = cudaMemPoolTrimTo(g_pool, 0);
+        if (first == cudaSuccess) first = e;
+    }
+    return (int)first;
 }
 
 int elpa2_bt_last_launch_count(void) { return g_last_launches; }

@@ -127,3 +127,7 @@ def test_launch_plan_invariants():
         assert pl["scratch_bytes"] > 0
     assert binding.plan(False, 1, 64, 10) == dict.fromkeys(("grid", "warps_per_cta", "P", "slabs", "slabs_per_cta_max",
                                                            "scratch_bytes"), 0)
+
+
+def test_release_scratch_without_anything_cached():
+    binding.release_scratch()          # nothing cached, no device needed: success

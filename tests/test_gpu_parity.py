@@ -209,3 +209,25 @@ def test_launch_on_side_stream():
         binding.trans_ev_tridi_to_band(N, nbw, dv, dt, q, stream=s)
     s.synchronize()
     assert np.abs(q.cpu().numpy() - want).max() <= TOL * np.abs(x).max()
+
+
+def test_release_scratch_and_reuse():
+    """The cached scratch can be handed back and the next calls allocate again."""
+    import torch
+
+    from paper_2002_10991_b200 import binding
+
+    before = torch.cuda.mem_get_info()[0]
+    _check(300, 64, 40, False)
+    N, nbw, nev = 260, 64, 45
+    hh_v, hh_tau, _, _ = _reflectors(N, nbw, 77, True)
+    x = _x(N, nev, 5, True)
+    y = np.array(x, order="F", copy=True)
+    binding.trans_ev_tridi_to_band_host(N, nbw, hh_v, hh_tau, y)
+    binding.release_scratch()
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] >= before - (64 << 20)       # nothing sizeable is held back
+    _check(300, 64, 40, True)                                          # and the library still works
+    y2 = np.array(x, order="F", copy=True)
+    binding.trans_ev_tridi_to_band_host(N, nbw, hh_v, hh_tau, y2)
+    assert np.array_equal(y, y2)
