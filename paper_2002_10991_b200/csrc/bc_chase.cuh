@@ -198,11 +198,16 @@ __global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, do
 // copies those segments into a tile S[col][row - r0] (column stride odd: conflict-free both ways),
 // runs the step there with exactly the arithmetic of bc_wavefront_kernel, and copies them back.
 template <int NBW>
-__device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
+__device__ __forceinline__ bool bc_step_smem(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
                                              double *__restrict__ hh_v, double *__restrict__ hh_tau, double *S, double *v,
                                              double *p, double *w2, double *sc, uint32_t *head_mine = nullptr,
-                                             const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
+                                             const uint32_t *head_prev = nullptr, const uint32_t need_head = 0,
+                                             const bool e_in = false, const bool allow_keep = false)
 {
+    // e_in: the previous step of this sweep left its block (iii) in S instead of writing it back -- it is
+    // this step's column x and block (i).  Returns true if this step does the same for the next one
+    // (allow_keep, persistent kernel only).  No other sweep reads that block in between: sweep s+1 needs
+    // it only after the next step has written it out, sweep s-1 shares just the corner, see below.
     constexpr int LG = (NBW == 32) ? 5 : 6;
     constexpr int64_t ldab = 2 * NBW + 1;
     constexpr int LDS = 2 * NBW + 1;              // tile column stride (doubles)
@@ -220,7 +225,7 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
             hh_tau[g] = 0.0;
             if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
         }
-        return;
+        return false;
     }
     int64_t r2 = r1 + NBW;
     if (r2 > N - 1) r2 = N - 1;
@@ -237,11 +242,32 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
             hi = nR;
         }
     };
-    // --- stage in: a warp per column, lanes along the column's contiguous band segment; cp.async keeps
-    //     every copy in flight at once (no index arithmetic worth mentioning: a flat (column, row) loop
-    //     spent more time on its divisions than on the copies)
+    // the next step's L is nR - L: keep block (iii) in S for it unless it is a one-row identity slot
+    const bool keep = allow_keep && (nR - L >= 2);
     const int warp = tid >> 5, lane = tid & 31, nwarp = nt >> 5;
-    for (int q = warp; q < ncol; q += nwarp) {
+    int qs = 0;                                   // first tile column to fetch from global memory
+    if (e_in) {
+        // previous step: L = NBW, its block (iii) sits at columns nAp .. nAp+NBW-1, rows NBW .. NBW+L-1
+        constexpr int MV = ((NBW - 1) * NBW + 255) / 256;
+        const int nAp = (k == 1) ? 0 : NBW - 1;
+        double tmp[MV];
+#pragma unroll
+        for (int m = 0; m < MV; ++m) {
+            const int idx = tid + m * 256, q = idx >> LG, row = idx & (NBW - 1);
+            tmp[m] = (q < NBW - 1 && row < L) ? S[(nAp + 1 + q) * LDS + NBW + row] : 0.0;
+        }
+        if (tid < L) p[tid] = S[nAp * LDS + NBW + tid];        // x = its first column
+        __syncthreads();
+#pragma unroll
+        for (int m = 0; m < MV; ++m) {
+            const int idx = tid + m * 256, q = idx >> LG, row = idx & (NBW - 1);
+            if (q < NBW - 1 && row < L) S[q * LDS + row] = tmp[m];
+        }
+        qs = nA;
+    }
+    // --- stage in: a warp per column, lanes along the column's contiguous band segment; cp.async keeps
+    //     every copy in flight at once
+    for (int q = qs + warp; q < ncol; q += nwarp) {
         int lo, hi;
         seg(q, lo, hi);
         const int64_t j = c + 1 + q;
@@ -250,7 +276,7 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
         for (int row = lo + lane; row < hi; row += 32) cp_async8(smem_u32(dst + row), src + row, 8u);
     }
     cp_async_commit();
-    if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];       // x = B[r0..r1][c]
+    if (!e_in && tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];       // x = B[r0..r1][c]
     cp_async_wait_all();
     __syncthreads();
 #define BS(rl, q) S[(q) * LDS + (rl)]
@@ -285,10 +311,10 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
         if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
     __syncthreads();
-    if (tau == 0.0) return;                       // the tile is unchanged: nothing to copy back
+    if (tau == 0.0 && !e_in) return false;        // the tile is unchanged and all of it is in global memory
     // Blocks (i), (ii), (iii) are disjoint and only read v: three groups of 64 threads run them side by
     // side; the two internal barriers of (ii) are named barriers of its own 64 threads.
-    const int grp = tid >> 6, t64 = tid & 63;
+    const int grp = (tau == 0.0) ? 3 : (tid >> 6), t64 = tid & 63;
     if (grp == 0) {
         // --- (i): one thread per column q < nA
         for (int q = t64; q < nA; q += 64) {
@@ -347,15 +373,17 @@ __device__ __forceinline__ void bc_step_smem(const int64_t N, const int64_t s, c
     }
     __syncthreads();
 #undef BS
-    // --- stage out
+    // --- stage out (block (iii) stays behind if the next step takes it from S)
     for (int q = warp; q < ncol; q += nwarp) {
         int lo, hi;
         seg(q, lo, hi);
+        if (keep && q >= nA) hi = L;
         const int64_t j = c + 1 + q;
         double *dst = ab + (r0 - j) + j * ldab;
         const double *src = S + q * LDS;
         for (int row = lo + lane; row < hi; row += 32) dst[row] = src[row];
     }
+    return keep;
 }
 
 // one launch per wavefront t = 3s + k
@@ -396,6 +424,7 @@ __global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *_
         const int64_t K = (N - 1 - s + NBW - 1) >> LG;
         const int64_t Kprev = (N - s + NBW - 1) >> LG;      // K(s-1)
         uint32_t known = 0;
+        bool e_in = false;                              // block (iii) of the previous step is still in S
         for (int64_t k = 0; k < K; ++k) {
             uint32_t need_head = 0;
             if (s > 0) {
@@ -409,7 +438,7 @@ __global__ void __launch_bounds__(256) bc_persistent_kernel(int64_t N, double *_
                 __syncthreads();
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);    // step (s-1, k+2) exists: its beta is our corner
             }
-            bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc, head + s, head + s - 1, need_head);
+            e_in = bc_step_smem<NBW>(N, s, k, ab, hh_v, hh_tau, S, v, p, w2, sc, head + s, head + s - 1, need_head, e_in, true);
             // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
             // barriers are built from): one fence, not one per thread
             __syncthreads();
