@@ -652,11 +652,12 @@ __global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__r
 // Two tiles: TA = block (i), nA columns x L rows (column stride NBW+1 elements); TB = blocks (ii)+(iii),
 // L columns x nR rows (column stride 2 NBW + 1): 198 KB at nbw = 64.  Arithmetic as bc_step_global_z.
 template <int NBW>
-__device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s, const int64_t k, zc *__restrict__ ab,
+__device__ __forceinline__ bool bc_step_smem_z(const int64_t N, const int64_t s, const int64_t k, zc *__restrict__ ab,
                                                zc *__restrict__ hh_v, zc *__restrict__ hh_tau, zc *TA, zc *TB, zc *v, zc *p,
                                                zc *w2, zc *zsc, double *dsc, uint32_t *head_mine,
-                                               const uint32_t *head_prev, const uint32_t need_head)
+                                               const uint32_t *head_prev, const uint32_t need_head, const bool e_in)
 {
+    // e_in / return value: block (iii) handed from step to step in shared memory, as in bc_step_smem
     constexpr int LG = (NBW == 32) ? 5 : 6;
     constexpr int64_t ldab = 2 * NBW + 1;
     constexpr int LDA = NBW + 1, LDB = 2 * NBW + 1;
@@ -674,14 +675,24 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
             hh_tau[g] = {0.0, 0.0};
             asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
         }
-        return;
+        return false;
     }
     int64_t r2 = r1 + NBW;
     if (r2 > N - 1) r2 = N - 1;
     const int nA = (int)(r0 - c - 1), nR = (int)(r2 - r0 + 1);
     // element (r0 + row, col j) of the band: ab[(r0 + row - j) + j * ldab]
+    const bool keep = (nR - L >= 2);              // the next step (L' = nR - L rows) takes block (iii) from TB
     const int warp = tid >> 5, lane = tid & 31, nwarp = nt >> 5;
-    for (int q = warp; q < nA + L; q += nwarp) {          // a warp per column, lanes along its band segment
+    int qs = 0;
+    if (e_in) {
+        // previous step: L = NBW; its block (iii) = TB rows NBW .. NBW+L-1: column 0 is x, columns 1.. block (i)
+        if (tid < L) p[tid] = TB[NBW + tid];
+        for (int q = warp; q < NBW - 1; q += nwarp)
+            for (int row = lane; row < L; row += 32) TA[q * LDA + row] = TB[(q + 1) * LDB + NBW + row];
+        __syncthreads();
+        qs = nA;
+    }
+    for (int q = qs + warp; q < nA + L; q += nwarp) {     // a warp per column, lanes along its band segment
         const int64_t j = c + 1 + q;
         const zc *src = ab + (r0 - j) + j * ldab;
         zc *dst = (q < nA) ? TA + q * LDA : TB + (q - nA) * LDB;
@@ -689,7 +700,7 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
         for (int row = lo + lane; row < hi; row += 32) cp_async16(smem_u32(dst + row), src + row, 16u);
     }
     cp_async_commit();
-    if (tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];
+    if (!e_in && tid < L) p[tid] = ab[(r0 + tid - c) + c * ldab];
     cp_async_wait_all();
     __syncthreads();
     if (tid == 0) {
@@ -725,10 +736,10 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
         asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
     __syncthreads();
-    if (ident) return;
+    if (ident && !e_in) return false;
 #define ZA(rl, q) TA[(q) * LDA + (rl)]
 #define ZB(rl, q) TB[(q) * LDB + (rl)]
-    const int grp = tid >> 6, t64 = tid & 63;
+    const int grp = ident ? 3 : (tid >> 6), t64 = tid & 63;
     if (grp == 0) {
         // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
         for (int q = t64; q < nA; q += 64) {
@@ -791,9 +802,10 @@ __device__ __forceinline__ void bc_step_smem_z(const int64_t N, const int64_t s,
         const int64_t j = c + 1 + q;
         zc *dst = ab + (r0 - j) + j * ldab;
         const zc *src = (q < nA) ? TA + q * LDA : TB + (q - nA) * LDB;
-        const int lo = (q < nA) ? 0 : q - nA, hi = (q < nA) ? L : nR;
+        const int lo = (q < nA) ? 0 : q - nA, hi = (q < nA) ? L : (keep ? L : nR);
         for (int row = lo + lane; row < hi; row += 32) dst[row] = src[row];
     }
+    return keep;
 }
 
 template <int NBW>
@@ -812,6 +824,7 @@ __global__ void __launch_bounds__(256) bc_persistent_smem_kernel_z(int64_t N, zc
         const int64_t K = (N - 1 - s + NBW - 1) >> LG;
         const int64_t Kprev = (N - s + NBW - 1) >> LG;
         uint32_t known = 0;
+        bool e_in = false;
         for (int64_t k = 0; k < K; ++k) {
             uint32_t need_head = 0;
             if (s > 0) {
@@ -824,7 +837,7 @@ __global__ void __launch_bounds__(256) bc_persistent_smem_kernel_z(int64_t N, zc
                 __syncthreads();
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
-            bc_step_smem_z<NBW>(N, s, k, ab, hh_v, hh_tau, TA, TB, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
+            e_in = bc_step_smem_z<NBW>(N, s, k, ab, hh_v, hh_tau, TA, TB, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head, e_in);
             // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
             // barriers are built from): one fence, not one per thread
             __syncthreads();
