@@ -56,6 +56,12 @@ def lib() -> ctypes.CDLL:
         for nm in ("orc_back_transform_d", "orc_back_transform_z"):
             getattr(_lib, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64]
             getattr(_lib, nm).restype = None
+        for nm in ("orc_full_to_band_d", "orc_full_to_band_z"):
+            getattr(_lib, nm).argtypes = [i64, i32, vp, i64, vp, i64, vp]
+            getattr(_lib, nm).restype = i32
+        for nm in ("orc_band_to_full_back_d", "orc_band_to_full_back_z"):
+            getattr(_lib, nm).argtypes = [i64, i32, i64, vp, i64, vp, vp, i64]
+            getattr(_lib, nm).restype = None
         _lib.orc_num_threads.argtypes = []
         _lib.orc_num_threads.restype = i32
     return _lib
@@ -139,6 +145,43 @@ def back_transform(N: int, nbw: int, hh_v: np.ndarray, hh_tau: np.ndarray, q: np
     ldq = q.strides[1] // q.itemsize if ncols > 1 else max(N, 1)
     fn = lib().orc_back_transform_z if cplx else lib().orc_back_transform_d
     fn(N, nbw, ncols, _p(hh_v), _p(hh_tau), _p(q), ldq)
+
+
+def full_to_band(a: np.ndarray, nbw: int):
+    """Eq. 6a (reading R15): reduce the full Hermitian matrix ``a`` (N x N, Fortran order, both
+    triangles) to a band of semi-bandwidth nbw, in place.  Returns (hv, tau): hv is N x Nv Fortran
+    order (column j = v_j at rows j+nbw.., unit head stored, zeros above), tau has Nv entries,
+    Nv = max(N - nbw - 1, 0)."""
+    cplx = np.iscomplexobj(a)
+    dt = np.complex128 if cplx else np.float64
+    assert a.dtype == dt and a.flags.f_contiguous and a.ndim == 2 and a.shape[0] == a.shape[1]
+    N = a.shape[0]
+    Nv = max(N - nbw - 1, 0)
+    hv = np.zeros((N, max(Nv, 1)), dtype=dt, order="F")[:, :Nv]
+    tau = np.zeros(Nv, dtype=dt)
+    fn = lib().orc_full_to_band_z if cplx else lib().orc_full_to_band_d
+    rc = fn(N, nbw, _p(a), max(N, 1), _p(hv), max(N, 1), _p(tau))
+    if rc != 0:
+        raise RuntimeError(f"orc_full_to_band failed: {rc}")
+    return hv, tau
+
+
+def band_to_full_back(N: int, nbw: int, hv: np.ndarray, tau: np.ndarray, q: np.ndarray) -> None:
+    """Eq. 6e: q <- H_0 H_1 ... H_{Nv-1} q in place (q Fortran-ordered N x ncols)."""
+    cplx = np.iscomplexobj(q)
+    dt = np.complex128 if cplx else np.float64
+    assert q.dtype == dt and hv.dtype == dt and tau.dtype == dt
+    assert q.ndim == 2 and q.shape[0] == N and q.strides[0] == q.itemsize
+    Nv = max(N - nbw - 1, 0)
+    assert hv.shape == (N, Nv) and tau.shape == (Nv,) and tau.flags.c_contiguous
+    if Nv == 0 or q.shape[1] == 0:
+        return
+    assert hv.strides[0] == hv.itemsize
+    ldv = hv.strides[1] // hv.itemsize if Nv > 1 else max(N, 1)
+    ncols = q.shape[1]
+    ldq = q.strides[1] // q.itemsize if ncols > 1 else max(N, 1)
+    fn = lib().orc_band_to_full_back_z if cplx else lib().orc_band_to_full_back_d
+    fn(N, nbw, ncols, _p(hv), ldv, _p(tau), _p(q), ldq)
 
 
 def num_threads() -> int:

@@ -19,6 +19,7 @@
  *   orc_tridiag_ql      : T X = X Lambda, X^T X = I; eigenvalues vs numpy.linalg.eigvalsh
  *   orc_back_transform_*: equals dense Q2 * X; X = I returns Q2; column norms preserved;
  *                         end-to-end ||B Y - Y Lambda|| / ||B|| <= 1e-12 N
+ *   orc_full_to_band_* / orc_band_to_full_back_* (Eqs. 6a, 6e): see the block comment above them
  *
  * Build: gcc -O2 -std=c99 -fopenmp -shared -fPIC -o libelpa2_oracle.so elpa2_oracle.c -lm
  * (no -ffast-math; OpenMP is used only to spread independent eigenvector columns,
@@ -467,4 +468,173 @@ int orc_num_threads(void)
     }
 #endif
     return n;
+}
+
+/* ==========================================================================================
+ * the steps around the band stage -- full -> band (Eq. 6a, PAPER.md:84:
+ * B = P H P*) and the band -> full back-transformation of the eigenvectors (Eq. 6e, PAPER.md:93:
+ * C = P* Y).  The paper gives the two equations and says 6a "mostly involves ... BLAS level-3
+ * matrix-matrix operations", nothing else; the reading taken here is DESIGN.md R15:
+ *
+ *   P* = H_0 H_1 ... H_{Nv-1},  Nv = max(N - nbw - 1, 0),  H_j = I - tau_j v_j v_j^H  (Eq. 7's form,
+ *   PAPER.md:121, with the larfg convention of R2/R7), where reflector j clears column j below the
+ *   band: it acts on rows j+nbw .. N-1 and is generated from H^(j)[j+nbw .. N-1][j], H^(j) being the
+ *   matrix after the first j two-sided updates  H <- H_j^H H H_j.
+ *
+ * A blocked (panel QR + trailing update) reduction produces the same reflectors up to rounding: the
+ * right-hand applications of H_j touch columns >= j+nbw only, i.e. never the other columns of the
+ * panel j belongs to, so deferring them changes nothing.  The oracle is therefore the plain unblocked
+ * definition, one reflector at a time on the full matrix, O(N^3): for tests at N <= ~1500.
+ *
+ * Reflector storage (the layout elpa2_trans_ev_band_to_full_* consumes, include/elpa2_bt.h):
+ *   hv: column-major N x Nv, leading dimension ldv >= N; column j holds v_j at rows j+nbw .. N-1
+ *   with hv[j+nbw + j*ldv] == 1 stored explicitly and rows < j+nbw ZERO;  tau[j], j < Nv.
+ *
+ * Pins (tests/test_oracle_full.py): dense Qf = H_0 .. H_{Nv-1} from textbook reflectors built in
+ * numpy gives Qf^H H Qf = B (band of semi-bandwidth nbw) and Qf^H Qf = I to 1e-13; eig(B) = eig(H);
+ * nbw = 1 equals LAPACK's one-stage tridiagonalization (scipy.linalg.hessenberg); nbw >= N-1 leaves H
+ * alone; back-transform = dense Qf * Y, Y = I returns Qf, column norms preserved, and end to end
+ * through 6a -> 6b -> 6c -> 6d -> 6e: || H C - C Lambda || / || H || <= 1e-12 N.
+ * ========================================================================================== */
+
+/* Eq. 6a.  a: N x N column-major (lda), full Hermitian storage (both triangles), overwritten with
+ * the band matrix B (both triangles; entries outside the band are set to exact zeros). */
+int orc_full_to_band_d(int64_t N, int nbw, double *a, int64_t lda, double *hv, int64_t ldv, double *tau)
+{
+    if (N < 0 || nbw < 1 || lda < (N > 1 ? N : 1)) return -1;
+    const int64_t Nv = (N - nbw - 1 > 0) ? N - nbw - 1 : 0;
+    double *x = malloc(sizeof(double) * (N > 0 ? N : 1)), *v = malloc(sizeof(double) * (N > 0 ? N : 1));
+    if (!x || !v) return -2;
+    for (int64_t j = 0; j < Nv; ++j) {
+        const int64_t r0 = j + nbw;
+        const int L = (int)(N - r0);
+        double t, beta;
+        for (int i = 0; i < L; ++i) x[i] = a[(r0 + i) + j * lda];
+        orc_larfg_d(L, x, v, &t, &beta);
+        for (int64_t i = 0; i < N; ++i) hv[i + j * ldv] = 0.0;
+        for (int i = 0; i < L; ++i) hv[(r0 + i) + j * ldv] = v[i];
+        tau[j] = t;
+        if (t != 0.0) {
+            /* A <- H^T A: rows r0.., every column */
+            for (int64_t c = 0; c < N; ++c) {
+                double dot = 0.0;
+                for (int i = 0; i < L; ++i) dot += v[i] * a[(r0 + i) + c * lda];
+                for (int i = 0; i < L; ++i) a[(r0 + i) + c * lda] -= t * v[i] * dot;
+            }
+            /* A <- A H: columns r0.., every row */
+            for (int64_t r = 0; r < N; ++r) {
+                double dot = 0.0;
+                for (int i = 0; i < L; ++i) dot += a[r + (r0 + i) * lda] * v[i];
+                for (int i = 0; i < L; ++i) a[r + (r0 + i) * lda] -= t * dot * v[i];
+            }
+        }
+        /* the eliminated entries are zero by construction, the head is beta */
+        a[r0 + j * lda] = beta;
+        a[j + r0 * lda] = beta;
+        for (int i = 1; i < L; ++i) {
+            a[(r0 + i) + j * lda] = 0.0;
+            a[j + (r0 + i) * lda] = 0.0;
+        }
+    }
+    free(x); free(v);
+    return 0;
+}
+
+int orc_full_to_band_z(int64_t N, int nbw, zdouble *a, int64_t lda, zdouble *hv, int64_t ldv, zdouble *tau)
+{
+    if (N < 0 || nbw < 1 || lda < (N > 1 ? N : 1)) return -1;
+    const int64_t Nv = (N - nbw - 1 > 0) ? N - nbw - 1 : 0;
+    zdouble *x = malloc(sizeof(zdouble) * (N > 0 ? N : 1)), *v = malloc(sizeof(zdouble) * (N > 0 ? N : 1));
+    if (!x || !v) return -2;
+    for (int64_t j = 0; j < Nv; ++j) {
+        const int64_t r0 = j + nbw;
+        const int L = (int)(N - r0);
+        zdouble t;
+        double beta;
+        for (int i = 0; i < L; ++i) x[i] = a[(r0 + i) + j * lda];
+        orc_larfg_z(L, x, v, &t, &beta);
+        for (int64_t i = 0; i < N; ++i) hv[i + j * ldv] = 0.0;
+        for (int i = 0; i < L; ++i) hv[(r0 + i) + j * ldv] = v[i];
+        tau[j] = t;
+        if (t != 0.0) {
+            const zdouble ct = conj(t);
+            /* A <- H^H A = A - conj(tau) v (v^H A) */
+            for (int64_t c = 0; c < N; ++c) {
+                zdouble dot = 0.0;
+                for (int i = 0; i < L; ++i) dot += conj(v[i]) * a[(r0 + i) + c * lda];
+                for (int i = 0; i < L; ++i) a[(r0 + i) + c * lda] -= ct * v[i] * dot;
+            }
+            /* A <- A H = A - tau (A v) v^H */
+            for (int64_t r = 0; r < N; ++r) {
+                zdouble dot = 0.0;
+                for (int i = 0; i < L; ++i) dot += a[r + (r0 + i) * lda] * v[i];
+                for (int i = 0; i < L; ++i) a[r + (r0 + i) * lda] -= t * dot * conj(v[i]);
+            }
+        }
+        a[r0 + j * lda] = beta;
+        a[j + r0 * lda] = beta;
+        for (int i = 1; i < L; ++i) {
+            a[(r0 + i) + j * lda] = 0.0;
+            a[j + (r0 + i) * lda] = 0.0;
+        }
+    }
+    for (int64_t i = 0; i < N; ++i) a[i + i * lda] = creal(a[i + i * lda]);   /* a Hermitian diagonal is real */
+    free(x); free(v);
+    return 0;
+}
+
+/* Eq. 6e: q <- P* q = H_0 (H_1 ( ... (H_{Nv-1} q))), the plain definition: the reflector generated
+ * last is applied first, each as x <- x - tau (v^H x) v on rows j+nbw .. N-1 (Eq. 8's form,
+ * PAPER.md:162; tau as stored, R2).  Columns are independent: OpenMP over column
+ * chunks, each thread running the whole reflector loop on its columns in exactly this order. */
+void orc_band_to_full_back_d(int64_t N, int nbw, int64_t ncols, const double *hv, int64_t ldv,
+                             const double *tau, double *q, int64_t ldq)
+{
+    const int64_t Nv = (N - nbw - 1 > 0) ? N - nbw - 1 : 0;
+    if (Nv == 0 || ncols < 1) return;
+    const int64_t chunk = orc_col_chunk(ncols);
+    const int64_t nchunks = (ncols + chunk - 1) / chunk;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t cb = 0; cb < nchunks; ++cb) {
+        int64_t j0 = cb * chunk, j1 = j0 + chunk < ncols ? j0 + chunk : ncols;
+        for (int64_t j = Nv - 1; j >= 0; --j) {
+            const double t = tau[j];
+            if (t == 0.0) continue;
+            const int64_t r0 = j + nbw, L = N - r0;
+            const double *v = hv + r0 + j * ldv;
+            for (int64_t c = j0; c < j1; ++c) {
+                double *x = q + r0 + c * ldq;
+                double dot = 0.0;
+                for (int64_t r = 0; r < L; ++r) dot += v[r] * x[r];
+                double td = t * dot;
+                for (int64_t r = 0; r < L; ++r) x[r] -= td * v[r];
+            }
+        }
+    }
+}
+
+void orc_band_to_full_back_z(int64_t N, int nbw, int64_t ncols, const zdouble *hv, int64_t ldv,
+                             const zdouble *tau, zdouble *q, int64_t ldq)
+{
+    const int64_t Nv = (N - nbw - 1 > 0) ? N - nbw - 1 : 0;
+    if (Nv == 0 || ncols < 1) return;
+    const int64_t chunk = orc_col_chunk(ncols);
+    const int64_t nchunks = (ncols + chunk - 1) / chunk;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t cb = 0; cb < nchunks; ++cb) {
+        int64_t j0 = cb * chunk, j1 = j0 + chunk < ncols ? j0 + chunk : ncols;
+        for (int64_t j = Nv - 1; j >= 0; --j) {
+            const zdouble t = tau[j];
+            if (t == 0.0) continue;
+            const int64_t r0 = j + nbw, L = N - r0;
+            const zdouble *v = hv + r0 + j * ldv;
+            for (int64_t c = j0; c < j1; ++c) {
+                zdouble *x = q + r0 + c * ldq;
+                zdouble dot = 0.0;
+                for (int64_t r = 0; r < L; ++r) dot += conj(v[r]) * x[r];
+                zdouble td = t * dot;
+                for (int64_t r = 0; r < L; ++r) x[r] -= td * v[r];
+            }
+        }
+    }
 }

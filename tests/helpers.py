@@ -29,3 +29,13 @@ def dense_reflector(N: int, r0: int, v: np.ndarray, tau) -> np.ndarray:
 
 def fortran(a: np.ndarray) -> np.ndarray:
     return np.array(a, order="F", copy=True)
+
+
+def band_from_dense(B: np.ndarray, nbw: int) -> np.ndarray:
+    """Lower band storage (2 nbw + 1, N), Fortran order, of a Hermitian band matrix given in full:
+    ab[i-j, j] = B[i, j] for 0 <= i-j <= nbw (rows nbw+1 .. 2 nbw stay zero: room for the chase)."""
+    N = B.shape[0]
+    ab = np.zeros((2 * nbw + 1, N), dtype=B.dtype, order="F")
+    for d in range(min(nbw, N - 1) + 1):
+        ab[d, : N - d] = np.diagonal(B, -d)
+    return ab
