@@ -77,9 +77,19 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
  *        fill and must be zero on entry).  Overwritten with the tridiagonal matrix T.
  *   hh_v (G*nbw), hh_tau (G): DEVICE outputs, every slot written (identity slots: v = e1, tau = 0).
  *   d (N), e (N-1): DEVICE outputs, diagonal and sub-diagonal of T = Q2^T B Q2.
- * Asynchronous on `stream`: about 3N kernel launches (one per wavefront 3s + k of independent
- * chase steps), no host synchronisation, no allocation.  Returns 0; -i for a bad i-th argument
- * (N=1, nbw=2, ab=3, hh_v=4, hh_tau=5, d=6, e=7); > 0 = cudaError_t.  N = 0: no work. */
+ * Asynchronous on `stream`, no host synchronisation.  Default schedule: ONE persistent kernel, launched
+ * cooperatively (every CTA of the grid -- one per SM -- must be resident at once, because sweeps hand
+ * over through per-sweep progress flags in global memory; the launch fails with a cudaError_t rather
+ * than deadlock if the device cannot hold the grid), plus one small kernel that extracts d and e.  Its
+ * 2N 32-bit progress counters come from the library's stream-ordered scratch pool (allocated, zeroed
+ * and freed in stream order; nothing new is allocated in steady state).  With ELPA2_BC_WAVEFRONT=1 in
+ * the environment (read once per process) the fallback schedule runs instead: one launch per wavefront
+ * t = 3s + k of independent chase steps, about 3N launches, stream order as the only dependency, no
+ * scratch.  Both schedules produce the same bits.
+ * Returns 0; -i for a bad i-th argument (N=1, nbw=2, ab=3, hh_v=4, hh_tau=5, d=6, e=7; a pointer that
+ * is NULL with work to do or not aligned to its element size -- 16 bytes for the complex call);
+ * > 0 = cudaError_t.  N = 0: no work.  The zero fill of rows nbw+1 .. 2*nbw of `ab` is the caller's
+ * duty and is not checked. */
 int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh_tau,
                         double *d, double *e, void *stream);
 /* Complex Hermitian (interleaved (re, im); the diagonal of B real): B <- H^H B H with the complex tau
@@ -88,14 +98,19 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau,
                         double *d, double *e, void *stream);
 
 /* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */
+/* Length L = min(nbw, N-1-s-k*nbw) of every slot in slot order (all but the last
+ * reflector of a sweep have length nbw): writes min(G, cap) entries to `out` (HOST, may be NULL to
+ * query) and returns G. */
+int64_t elpa2_hh_lengths(int64_t N, int nbw, int32_t *out, int64_t cap);
 int64_t elpa2_hh_count(int64_t N, int nbw);
 /* first slot of sweep s (s in [0, N-1]; s = N-1 gives G); -1 if out of range */
 int64_t elpa2_hh_offset(int64_t N, int nbw, int64_t s);
 /* K(s), 0 if s is out of range */
 int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
 
-/* Kernels launched by the last successful compute call of this thread's library state (for
- * bench.py's "gpu_launches"), and a selector for A/B runs: variant 0 = default (compact-WY
+/* Kernels launched by the last successful compute call of the calling thread (for bench.py's
+ * "gpu_launches"), and a selector for A/B runs.  Both are per thread: elpa2_bt_set_variant changes what
+ * later calls (and elpa2_bt_plan) of the SAME thread do and nothing else.  Variants: variant 0 = default (compact-WY
  * aggregation of 8 reflectors on the FP64 tensor cores, R6: a T-factor prepass kernel + the main
  * kernel = 2 launches; its scratch comes from a stream-ordered pool that keeps its memory),
  * 1 = plain kernel (one thread per column, literal reverse generation order), 2 = one reflector at

@@ -22,6 +22,7 @@ EXPORTS = (
     "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
     "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
+    "elpa2_hh_lengths",
 )
 
 
@@ -64,6 +65,8 @@ def lib() -> ctypes.CDLL:
         L.elpa2_hh_offset.restype = i64
         L.elpa2_hh_blocks.argtypes = [i64, i32, i64]
         L.elpa2_hh_blocks.restype = i32
+        L.elpa2_hh_lengths.argtypes = [i64, i32, vp, i64]
+        L.elpa2_hh_lengths.restype = i64
         L.elpa2_bt_last_launch_count.argtypes = []
         L.elpa2_bt_last_launch_count.restype = i32
         L.elpa2_bt_set_variant.argtypes = [i32]
@@ -96,17 +99,15 @@ def hh_blocks(N: int, nbw: int, s: int) -> int:
 
 
 def hh_lengths(N: int, nbw: int):
-    """Length L of every reflector slot, in slot order (int64 numpy array of G entries), built
-    from the library's own layout helpers: slot (s, k) has L = min(nbw, N-1-s-k*nbw)."""
+    """Length L of every reflector slot, in slot order (int32 numpy array of G entries), from the
+    library's ``elpa2_hh_lengths``."""
     import numpy as np
 
-    if N < 2:
-        return np.zeros(0, dtype=np.int64)
-    K = np.array([hh_blocks(N, nbw, s) for s in range(N - 1)], dtype=np.int64)
-    s_of_g = np.repeat(np.arange(N - 1, dtype=np.int64), K)
-    first = np.cumsum(K) - K
-    k_of_g = np.arange(int(K.sum()), dtype=np.int64) - np.repeat(first, K)
-    return np.minimum(nbw, N - 1 - s_of_g - k_of_g * nbw)
+    G = max(int(lib().elpa2_hh_lengths(N, nbw, None, 0)), 0)
+    out = np.zeros(G, dtype=np.int32)
+    if G:
+        lib().elpa2_hh_lengths(N, nbw, out.ctypes.data, G)
+    return out
 
 
 def plan(cplx: bool, N: int, nbw: int, nev: int, n_sm: int = 148) -> dict:
@@ -178,6 +179,13 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
     ldq = q.stride(1) if nev > 1 else max(N, 1)
     if not (hh_v.is_contiguous() and hh_tau.is_contiguous()):
         raise ValueError("hh_v / hh_tau must be contiguous")
+    G = hh_count(N, nbw)
+    if G > 0 and (tuple(hh_v.shape) != (G, nbw) or tuple(hh_tau.shape) != (G,)):
+        raise ValueError(f"hh_v must be ({G}, {nbw}) and hh_tau ({G},) for N = {N}, nbw = {nbw}")
+    if not (hh_v.device == q.device and hh_tau.device == q.device):
+        raise ValueError("hh_v, hh_tau and q must live on the same device")
+    if torch.cuda.current_device() != q.device.index:
+        raise ValueError("q's device must be the current CUDA device")
     rc = trans_ev_tridi_to_band_raw(cplx, N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q.data_ptr(),
                                     ldq, _stream_ptr(stream))
     if rc != 0:
@@ -187,7 +195,7 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
 def bulge_chase(N: int, nbw: int, ab, stream=None):
     """Band -> tridiagonal on the device (Eq. 6b).  ``ab``: CUDA float64 / complex128 tensor of shape
     (N, 2*nbw+1), row j = column j of the lower band storage (ab[j, i-j] = B[i, j]), overwritten
-    with T.  Returns CUDA tensors (hh_v (G, nbw), hh_tau (G,), d (N,), e (N-1,)); d, e are real."""
+    with T.  Entries ab[:, nbw+1:] are room for the fill and MUST be zero on entry (not checked).  Returns CUDA tensors (hh_v (G, nbw), hh_tau (G,), d (N,), e (N-1,)); d, e are real."""
     import torch
 
     if (not ab.is_cuda or ab.dtype not in (torch.float64, torch.complex128) or not ab.is_contiguous()

@@ -315,7 +315,19 @@ __device__ __forceinline__ bool bc_step_smem(const int64_t N, const int64_t s, c
     // Blocks (i), (ii), (iii) are disjoint and only read v: three groups of 64 threads run them side by
     // side; the two internal barriers of (ii) are named barriers of its own 64 threads.
     const int grp = (tau == 0.0) ? 3 : (tid >> 6), t64 = tid & 63;
-    if (grp == 0) {
+    if (grp == 3) {
+        // identity step that goes on because it holds the previous step's block (iii): nothing to compute,
+        // but the corner staged in above may predate the beta of step (s-1, k+2) -- it must not be staged
+        // out (or handed on) stale.  Same wait and re-fetch as group 1 below.
+        if (need_head && tid == 0 && nR > L) {
+            uint32_t h;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+            } while (h < need_head);
+            const int64_t jc = c + 1 + (nA + L - 1);
+            BS(nR - 1, nA + L - 1) = __ldcg(&ab[(r0 + nR - 1 - jc) + jc * ldab]);
+        }
+    } else if (grp == 0) {
         // --- (i): one thread per column q < nA
         for (int q = t64; q < nA; q += 64) {
             double dot = 0.0;
@@ -740,7 +752,19 @@ __device__ __forceinline__ bool bc_step_smem_z(const int64_t N, const int64_t s,
 #define ZA(rl, q) TA[(q) * LDA + (rl)]
 #define ZB(rl, q) TB[(q) * LDB + (rl)]
     const int grp = ident ? 3 : (tid >> 6), t64 = tid & 63;
-    if (grp == 0) {
+    if (grp == 3) {
+        // identity step holding the previous step's block (iii): re-fetch the corner once step (s-1, k+2)
+        // has written its beta there, as group 1 does (see bc_step_smem)
+        if (need_head && tid == 0 && nR > L) {
+            uint32_t h;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+            } while (h < need_head);
+            const int64_t jc = r0 + L - 1;
+            const double2 cv = __ldcg(reinterpret_cast<const double2 *>(&ab[(r0 + nR - 1 - jc) + jc * ldab]));
+            ZB(nR - 1, L - 1) = {cv.x, cv.y};
+        }
+    } else if (grp == 0) {
         // --- (i) A <- H^H A = A - conj(tau) v (v^H A)
         for (int q = t64; q < nA; q += 64) {
             zc dot = {0.0, 0.0};
@@ -886,13 +910,8 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     int64_t nl = 0;
     constexpr int smem_bytes = (2 * NBW - 1) * (2 * NBW + 1) * 8;
     if (NBW <= 64) {
-        static bool attr_done = false;
-        if (!attr_done) {
-            cudaError_t e0 = cudaFuncSetAttribute(bc_wavefront_smem_kernel<(NBW <= 64 ? NBW : 64)>,
-                                                  cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-            if (e0 != cudaSuccess) return e0;
-            attr_done = true;
-        }
+        cudaError_t e0 = set_max_smem((const void *)bc_wavefront_smem_kernel<(NBW <= 64 ? NBW : 64)>, smem_bytes);
+        if (e0 != cudaSuccess) return e0;
     }
     if (NBW > 64 && prog && nsm > 0 && N >= 2) {
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
@@ -901,12 +920,8 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
         if (e1 != cudaSuccess) return e1;
     } else if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
         auto pk = bc_persistent_kernel<(NBW <= 64 ? NBW : 64)>;
-        static bool pattr_done = false;
-        if (!pattr_done) {
-            cudaError_t e0 = cudaFuncSetAttribute(pk, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_bytes);
-            if (e0 != cudaSuccess) return e0;
-            pattr_done = true;
-        }
+        cudaError_t e0 = set_max_smem((const void *)pk, smem_bytes);
+        if (e0 != cudaSuccess) return e0;
         // one CTA per SM (its tile takes more than half of an SM's shared memory): all CTAs are resident,
         // which the flag waits between sweeps rely on
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
@@ -961,12 +976,8 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
             constexpr int NB = (NBW <= 64) ? NBW : 64;
             constexpr int zbytes = ((NB - 1) * (NB + 1) + NB * (2 * NB + 1)) * 16;
             auto zk = bc_persistent_smem_kernel_z<NB>;
-            static bool zattr = false;
-            if (!zattr) {
-                cudaError_t e0 = cudaFuncSetAttribute(zk, cudaFuncAttributeMaxDynamicSharedMemorySize, zbytes);
-                if (e0 != cudaSuccess) return e0;
-                zattr = true;
-            }
+            cudaError_t e0 = set_max_smem((const void *)zk, zbytes);
+            if (e0 != cudaSuccess) return e0;
             e1 = bc_launch_persistent(zk, grid, 256, zbytes, st, N, ab, hh_v, hh_tau, prog);
         } else
             e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 384, 0, st, N, ab, hh_v, hh_tau, prog);

@@ -18,6 +18,14 @@ __host__ __device__ __forceinline__ int64_t hh_off(int64_t N, int lg, int64_t s)
     return hh_F(N - 1, lg) - hh_F(N - 1 - s, lg);
 }
 
+// Opt-in to more than 48 KB of dynamic shared memory.  The attribute belongs to the (function, device)
+// pair, so it is set on every launch path call (a host-side table lookup in the runtime, no device
+// work) instead of once per process: a second device in the same process gets it too.
+inline cudaError_t set_max_smem(const void *func, int bytes)
+{
+    return cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+}
+
 // ---- kernel arguments of the window kernels ------------------------------------------------------
 struct WinArgs {
     int64_t N, nev, ldq;

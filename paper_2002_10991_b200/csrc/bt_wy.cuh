@@ -569,11 +569,9 @@ cudaError_t launch_wy_main(const WyArgs &a, const WyPlan &pl, cudaStream_t st)
 {
     using C = WyCfg<NBW, NWARPS>;
     auto kern = bt_wy_kernel<NBW, NWARPS>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    {
+        cudaError_t e = set_max_smem((const void *)kern, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     kern<<<(unsigned)pl.grid, NWARPS * 32, C::SMEM_BYTES, st>>>(a);
     return cudaGetLastError();

@@ -452,11 +452,9 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
 {
     using C = WyzCfg<NBW>;
     auto kern = bt_wyz_kernel<NBW>;
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, C::SMEM_BYTES);
+    {
+        cudaError_t e = set_max_smem((const void *)kern, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     const int64_t K0 = wy_nchains(N, C::LG);
     const int64_t nslab = (nev + 7) >> 3;

@@ -7,6 +7,7 @@
 
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdlib>
 #include <mutex>
 
@@ -24,25 +25,33 @@ using namespace elpa2bt;
 
 namespace {
 
-int g_variant = 0;
+// library state is per calling thread (variant selector, launch counter) or per device (SM count,
+// scratch pool, kernel attributes): no call changes what another thread's or another device's call does
+thread_local int g_variant = 0;
 thread_local int g_last_launches = 0;
+constexpr int MAX_DEV = 64;
 std::mutex g_mu;        // host-buffer entry point (its cached device scratch)
 std::mutex g_pool_mu;   // creation of the scratch pool
 
 int lg_of(int nbw) { return nbw == 32 ? 5 : nbw == 64 ? 6 : nbw == 128 ? 7 : -1; }
 
+int current_device()
+{
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= MAX_DEV) return 0;
+    return dev;
+}
+
 int sm_count()
 {
-    static int n = 0;
-    if (n == 0) {
-        int dev = 0, v = 0;
-        if (cudaGetDevice(&dev) == cudaSuccess &&
-            cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && v > 0)
-            n = v;
-        else
-            return 148;
+    static std::atomic<int> n[MAX_DEV];
+    const int dev = current_device();
+    int v = n[dev].load(std::memory_order_relaxed);
+    if (v == 0) {
+        if (cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || v <= 0) return 148;
+        n[dev].store(v, std::memory_order_relaxed);
     }
-    return n;
+    return v;
 }
 
 // the shift kernel: 7 consumer warps + 1 producer warp = 256 threads, so that each thread may use
@@ -54,13 +63,10 @@ cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const doubl
     using C = ShiftCfg<CPLX, NBW, CPL>;
     constexpr int MAXT = 256;
     auto kern = bt_shift_kernel<CPLX, NBW, CPL, MAXT, ELPA2_BT_UNROLL>;
-    static bool attr_done = false;
     constexpr int NWMAX = MAXT / 32 - 1;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)C::smem_bytes(NWMAX));
+    {
+        cudaError_t e = set_max_smem((const void *)kern, (int)C::smem_bytes(NWMAX));
         if (e != cudaSuccess) return e;
-        attr_done = true;
     }
     const int64_t units = (nev + C::CW - 1) / C::CW;
     const int64_t nsm = sm_count();
@@ -84,18 +90,20 @@ cudaError_t launch_shift(int64_t N, int64_t nev, const double *hh_v, const doubl
 // stream-ordered scratch for the -T factors of the WY kernel: a private memory pool that keeps
 // what it has allocated (release threshold = max), so that in steady state a call allocates
 // nothing new and never synchronises the host
-cudaMemPool_t g_pool = nullptr;     // written under g_pool_mu
-int g_pool_dev = -1;
+cudaMemPool_t g_pool[MAX_DEV] = {};     // one per device, written under g_pool_mu
 
 cudaMemPool_t scratch_pool(cudaError_t *err)
 {
-    cudaMemPool_t &pool = g_pool;
-    int &pool_dev = g_pool_dev;
     int dev = 0;
     *err = cudaGetDevice(&dev);
     if (*err != cudaSuccess) return nullptr;
+    if (dev < 0 || dev >= MAX_DEV) {
+        *err = cudaErrorInvalidDevice;
+        return nullptr;
+    }
     std::lock_guard<std::mutex> lock(g_pool_mu);
-    if (pool && pool_dev == dev) return pool;
+    cudaMemPool_t &pool = g_pool[dev];
+    if (pool) return pool;
     cudaMemPoolProps props = {};
     props.allocType = cudaMemAllocationTypePinned;
     props.handleTypes = cudaMemHandleTypeNone;
@@ -107,7 +115,6 @@ cudaMemPool_t scratch_pool(cudaError_t *err)
     uint64_t keep = UINT64_MAX;
     cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
     pool = p;
-    pool_dev = dev;
     return pool;
 }
 
@@ -268,6 +275,9 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
     if (N >= 2 && !hh_tau) return -5;
     if (!d) return -6;
     if (N >= 2 && !e) return -7;
+    if (((uintptr_t)ab & 7) != 0) return -3;
+    if (((uintptr_t)hh_v & 7) != 0) return -4;
+    if (((uintptr_t)hh_tau & 7) != 0) return -5;
     cudaStream_t st = (cudaStream_t)stream;
     int64_t nl = 0;
     cudaError_t err;
@@ -279,7 +289,10 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
         cudaMemPool_t pool = scratch_pool(&err);
         if (!pool) return (int)err;
         if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)2 * N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
-        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) return (int)err;
+        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) {
+            cudaFreeAsync(prog, st);
+            return (int)err;
+        }
     }
     switch (nbw) {
     case 32: err = launch_bulge_chase<32>(N, ab, hh_v, hh_tau, d, e, st, &nl, prog, sm_count()); break;
@@ -306,6 +319,10 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, 
     if (N >= 2 && !hh_tau) return -5;
     if (!d) return -6;
     if (N >= 2 && !e) return -7;
+    // interleaved complex elements are moved 16 bytes at a time (cp.async 16, 128-bit loads)
+    if (((uintptr_t)ab & 15) != 0) return -3;
+    if (((uintptr_t)hh_v & 15) != 0) return -4;
+    if (((uintptr_t)hh_tau & 15) != 0) return -5;
     cudaStream_t st = (cudaStream_t)stream;
     int64_t nl = 0;
     cudaError_t err;
@@ -315,7 +332,10 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, 
         cudaMemPool_t pool = scratch_pool(&err);
         if (!pool) return (int)err;
         if ((err = cudaMallocFromPoolAsync((void **)&prog, (size_t)2 * N * sizeof(uint32_t), pool, st)) != cudaSuccess) return (int)err;
-        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) return (int)err;
+        if ((err = cudaMemsetAsync(prog, 0, (size_t)2 * N * sizeof(uint32_t), st)) != cudaSuccess) {
+            cudaFreeAsync(prog, st);
+            return (int)err;
+        }
     }
     switch (nbw) {
     case 32: err = launch_bulge_chase_z<32>(N, (zc *)ab, (zc *)hh_v, (zc *)hh_tau, d, e, st, &nl, prog, sm_count()); break;
@@ -350,6 +370,24 @@ int elpa2_hh_blocks(int64_t N, int nbw, int64_t s)
     const int lg = lg_of(nbw);
     if (lg < 0 || N < 2 || s < 0 || s > N - 2) return 0;
     return (int)((N - 1 - s + nbw - 1) >> lg);
+}
+
+int64_t elpa2_hh_lengths(int64_t N, int nbw, int32_t *out, int64_t cap)
+{
+    const int lg = lg_of(nbw);
+    if (lg < 0 || N < 2) return 0;
+    const int64_t G = hh_F(N - 1, lg);
+    if (!out) return G;
+    int64_t g = 0;
+    for (int64_t s = 0; s <= N - 2; ++s) {
+        const int64_t K = (N - 1 - s + nbw - 1) >> lg;
+        for (int64_t k = 0; k < K; ++k, ++g) {
+            if (g >= cap) return G;
+            const int64_t rest = N - 1 - s - k * nbw;      // rows r0 .. N-1
+            out[g] = (int32_t)(rest < nbw ? rest : nbw);
+        }
+    }
+    return G;
 }
 
 int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int64_t out[6])
@@ -393,10 +431,11 @@ int elpa2_bt_release_scratch(void)
         }
     }
     std::lock_guard<std::mutex> lock(g_pool_mu);
-    if (g_pool) {
-        const cudaError_t e = cudaMemPoolTrimTo(g_pool, 0);
-        if (first == cudaSuccess) first = e;
-    }
+    for (int dev = 0; dev < MAX_DEV; ++dev)
+        if (g_pool[dev]) {
+            const cudaError_t e = cudaMemPoolTrimTo(g_pool[dev], 0);
+            if (first == cudaSuccess) first = e;
+        }
     return (int)first;
 }
 

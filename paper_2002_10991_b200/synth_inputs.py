@@ -63,6 +63,58 @@ def band_matrix(N: int, nbw: int, seed: int, cplx: bool = False) -> np.ndarray:
     return ab
 
 
+def dense_hermitian(N: int, seed: int, cplx: bool = False) -> np.ndarray:
+    """Full N x N symmetric / Hermitian matrix (Fortran order, both triangles) with lower-triangle
+    entries hashed uniform in [-1, 1) (complex: both parts) and a real diagonal -- the "randomly
+    generated" matrices of PAPER.md:196 before the full -> band reduction."""
+    ii, jj = np.meshgrid(np.arange(N, dtype=np.uint64), np.arange(N, dtype=np.uint64), indexing="ij")
+    lo, hi = np.minimum(ii, jj), np.maximum(ii, jj)
+    ctr = hi * np.uint64(max(N, 1)) + lo
+    re = hash_uniform(seed, ctr, 0)
+    if cplx:
+        im = hash_uniform(seed, ctr, 1)
+        im = np.where(ii > jj, im, np.where(ii < jj, -im, 0.0))
+        a = re + 1j * im
+    else:
+        a = re
+    return np.asfortranarray(a)
+
+
+def structured_band_matrix(N: int, nbw: int, seed: int, cplx: bool, kind: str) -> np.ndarray:
+    """Degenerate variants of ``band_matrix`` (same storage) that make the chase produce identity
+    reflectors in the middle of a chain -- the inputs a KS-DFT matrix with decoupled blocks or a
+    narrower true band gives:
+
+    * ``blockdiag``: couplings across the cuts at rows 20, N//2 and N//2 + nbw + 3 are zero
+    * ``narrow2`` / ``narrow1``: true semi-bandwidth nbw//2 / 1 (already tridiagonal)
+    * ``zero``, ``identity``: the zero matrix, the unit matrix
+    * ``zerotail``: the last N//3 columns have no off-diagonal entries
+    * ``sparsecols``: every third column has no off-diagonal entries
+    """
+    ab = band_matrix(N, nbw, seed, cplx)
+    jj, dd = np.meshgrid(np.arange(N), np.arange(2 * nbw + 1))
+    ii = jj + dd
+    if kind == "blockdiag":
+        for cut in (20, N // 2, N // 2 + nbw + 3):
+            ab[(ii >= cut) & (jj < cut)] = 0.0
+    elif kind == "narrow2":
+        ab[dd > nbw // 2] = 0.0
+    elif kind == "narrow1":
+        ab[dd > 1] = 0.0
+    elif kind == "zero":
+        ab[:] = 0.0
+    elif kind == "identity":
+        ab[:] = 0.0
+        ab[0, :] = 1.0
+    elif kind == "zerotail":
+        ab[(dd > 0) & (jj >= N - N // 3)] = 0.0
+    elif kind == "sparsecols":
+        ab[(dd > 0) & (jj % 3 == 1)] = 0.0
+    else:
+        raise ValueError(kind)
+    return ab
+
+
 def sample_columns(nev: int, count: int, seed: int) -> np.ndarray:
     """``count`` distinct column indices of [0, nev), seeded, sorted."""
     rng = np.random.default_rng(seed)

@@ -42,6 +42,40 @@ def test_layout_helpers_match_oracle(lib, N, nbw):
         assert binding.hh_blocks(N, nbw, N - 1) == 0
 
 
+@pytest.mark.parametrize("N,nbw", [(2, 32), (17, 32), (33, 32), (100, 64), (130, 128), (515, 64), (1000, 32)])
+def test_hh_lengths_match_oracle_rows(lib, N, nbw):
+    """elpa2_hh_lengths (the only place the binding gets slot lengths from) against the oracle's
+    row map, which the paper's worked example pins (tests/test_oracle_layout.py)."""
+    got = binding.hh_lengths(N, nbw)
+    want = [orc.hh_rows(N, nbw, s, k)[2] for s in range(N - 1) for k in range(orc.hh_blocks(N, nbw, s))]
+    assert got.tolist() == want
+    assert int(got.sum()) == N * (N - 1) // 2          # sum of L = N(N-1)/2 (SURVEY 7.2)
+    assert lib.elpa2_hh_lengths(N, nbw, None, 0) == len(want)
+
+
+def test_variant_selector_is_per_thread(lib):
+    """elpa2_bt_set_variant in one thread changes neither another thread's variant nor its plan."""
+    import threading
+
+    args = (False, 4096, 64, 32768, 148)
+    base = binding.plan(*args)
+    assert binding.set_variant(0) == 0
+    seen = {}
+
+    def other():
+        seen["old"] = binding.set_variant(3)          # this thread starts at the default, 0
+        seen["plan3"] = binding.plan(*args)
+        seen["now"] = binding.set_variant(3)
+
+    t = threading.Thread(target=other)
+    t.start()
+    t.join()
+    assert seen["old"] == 0 and seen["now"] == 3
+    assert seen["plan3"]["P"] == 2                     # variant 3: two chains per pass
+    assert binding.plan(*args) == base and base["P"] == 1
+    assert binding.set_variant(0) == 0                 # still the default here
+
+
 def test_layout_full_size_counts(lib):
     # SURVEY.md 8(a) table: G for the five configs
     assert binding.hh_count(512, 32) == 4336
