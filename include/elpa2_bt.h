@@ -97,6 +97,25 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
 int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau,
                         double *d, double *e, void *stream);
 
+/* the band -> full back-transformation of the eigenvectors, Eq. 6e (PAPER.md:93,
+ * C = P* Y; PAPER.md:232, :302 name it a target for further optimisation).  The paper states the
+ * equation only; R15 is the reading: P* = H_0 H_1 ... H_{Nv-1}, Nv = max(N - nbw - 1, 0), where
+ * H_j = I - tau_j v_j v_j^H is the reflector that cleared column j below the band in the full -> band
+ * reduction (Eq. 6a) and acts on rows j+nbw .. N-1.  The call overwrites
+ *
+ *      q  <-  H_0 ( H_1 ( ... ( H_{Nv-1} q ) ) )        (the reflector generated last is applied first)
+ *
+ * tau as stored (R2).  Layout: hv is column-major N x Nv with leading dimension ldv (ldv >= N, ldv even,
+ * hv 16-byte aligned): column j holds v_j at rows j+nbw .. N-1, the unit head hv[j+nbw + j*ldv] == 1
+ * stored explicitly, rows < j+nbw ZERO (the kernel multiplies whole tiles); tau[j], j < Nv.
+ * q as above (N x nev, column-major, ldq).  All DEVICE pointers; asynchronous on `stream`; the -T factors
+ * of the blocks of 64 reflectors (32 KB each) come from the library's stream-ordered scratch pool.
+ * nbw: any positive multiple of 16.  Two launches (T-factor prepass + the fused DMMA kernel).
+ * Returns 0; -i for a bad i-th argument (N=1, nbw=2, nev=3, hv=4, ldv=5, tau=6, q=7, ldq=8); > 0 = cudaError_t.
+ * Nv == 0 or nev == 0: success, no work. */
+int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv,
+                                  const double *tau, double *q, int64_t ldq, void *stream);
+
 /* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */
 /* Length L = min(nbw, N-1-s-k*nbw) of every slot in slot order (all but the last
  * reflector of a sweep have length nbw): writes min(G, cap) entries to `out` (HOST, may be NULL to

@@ -22,7 +22,7 @@ EXPORTS = (
     "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
     "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
-    "elpa2_hh_lengths",
+    "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d",
 )
 
 
@@ -55,6 +55,8 @@ def lib() -> ctypes.CDLL:
         for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
             getattr(L, nm).argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
             getattr(L, nm).restype = i32
+        L.elpa2_trans_ev_band_to_full_d.argtypes = [i64, i32, i64, vp, i64, vp, vp, i64, vp]
+        L.elpa2_trans_ev_band_to_full_d.restype = i32
         L.elpa2_bt_release_scratch.argtypes = []
         L.elpa2_bt_release_scratch.restype = i32
         L.elpa2_bt_plan.argtypes = [i32, i64, i32, i64, i32, ctypes.POINTER(i64)]
@@ -180,7 +182,7 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
     if not (hh_v.is_contiguous() and hh_tau.is_contiguous()):
         raise ValueError("hh_v / hh_tau must be contiguous")
     G = hh_count(N, nbw)
-    if G > 0 and (tuple(hh_v.shape) != (G, nbw) or tuple(hh_tau.shape) != (G,)):
+    if G > 0 and nev > 0 and (tuple(hh_v.shape) != (G, nbw) or tuple(hh_tau.shape) != (G,)):
         raise ValueError(f"hh_v must be ({G}, {nbw}) and hh_tau ({G},) for N = {N}, nbw = {nbw}")
     if not (hh_v.device == q.device and hh_tau.device == q.device):
         raise ValueError("hh_v, hh_tau and q must live on the same device")
@@ -188,6 +190,32 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
         raise ValueError("q's device must be the current CUDA device")
     rc = trans_ev_tridi_to_band_raw(cplx, N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q.data_ptr(),
                                     ldq, _stream_ptr(stream))
+    if rc != 0:
+        raise Elpa2BtError(rc)
+
+
+def trans_ev_band_to_full(N: int, nbw: int, hv, tau, q, stream=None) -> None:
+    """q <- P* q in place (Eq. 6e).  ``hv``: CUDA tensor of shape (N, Nv) stored column-major
+    (``hv.stride(0) == 1``, ldv = ``hv.stride(1)``), Nv = max(N - nbw - 1, 0); ``tau`` (Nv,); ``q`` (N, nev)
+    column-major.  Layout per include/elpa2_bt.h."""
+    import torch
+
+    if not (q.is_cuda and hv.is_cuda and tau.is_cuda):
+        raise ValueError("device tensors required")
+    if q.dtype != torch.float64 or hv.dtype != q.dtype or tau.dtype != q.dtype:
+        raise ValueError("float64 throughout")
+    Nv = max(N - nbw - 1, 0)
+    if q.dim() != 2 or q.shape[0] != N or (N > 1 and q.stride(0) != 1):
+        raise ValueError("q must be (N, nev) column-major")
+    nev = q.shape[1]
+    ldq = q.stride(1) if nev > 1 else max(N, 1)
+    if Nv > 0 and (tuple(hv.shape) != (N, Nv) or hv.stride(0) != 1 or tuple(tau.shape) != (Nv,) or not tau.is_contiguous()):
+        raise ValueError(f"hv must be ({N}, {Nv}) column-major and tau ({Nv},)")
+    ldv = hv.stride(1) if Nv > 1 else max(N + (N & 1), 2)
+    if not (hv.device == q.device and tau.device == q.device and torch.cuda.current_device() == q.device.index):
+        raise ValueError("hv, tau and q must live on the current CUDA device")
+    rc = lib().elpa2_trans_ev_band_to_full_d(N, nbw, nev, hv.data_ptr(), ldv, tau.data_ptr(), q.data_ptr(), ldq,
+                                             _stream_ptr(stream))
     if rc != 0:
         raise Elpa2BtError(rc)
 

@@ -1,0 +1,468 @@
+// bt_b2f.cuh -- SURVEY.md 8(f) NEXT-2: band -> full back-transformation of the eigenvectors (Eq. 6e,
+// C = P* Y) on the FP64 tensor cores (DMMA m8n8k4), real FP64, sm_100a.
+// What it computes: include/elpa2_bt.h, reading R15 of DESIGN.md:
+//      q <- H_0 H_1 ... H_{Nv-1} q,   H_j = I - tau_j v_j v_j^T on rows j+nbw .. N-1,  Nv = N - nbw - 1.
+// The paper names this step a BLAS-3 (cuBLAS) step and, with 6a, "the first target for further ...
+// optimization".  Here it is ONE hand-written GEMM-class kernel, not a sequence of
+// library GEMMs:
+//
+//  * Blocks of NB = 64 consecutive reflectors, Q_p = H_{64p} .. H_{64p+63} = I - V_p T_p V_p^T (compact
+//    WY, T_p upper triangular: T[i][i] = tau_i, T[:i, i] = -tau_i T[:i,:i] (V[:, :i]^T v_i); the prepass
+//    kernel b2f_tfactor_kernel writes -T_p).  q <- Q_0 (Q_1 ( .. Q_{npb-1} q)): block npb-1 first.
+//  * Applying Q_p is  W = V_p^T q  (64 x cols, K = rows),  U = (-T_p) W,  q += V_p U  (K = 64).  The two
+//    big products of CONSECUTIVE blocks are fused into one pass over q ("look-ahead"): pass P reads a
+//    16-row group of q once, updates it with block P (q += V_P U_P), feeds the updated rows straight
+//    into the dot product of block P-1 (W_{P-1} += V_{P-1}^T q) and writes it once.  q traffic per
+//    block is one read + one write instead of two reads + one write: 2*8 bytes per 4*64 flops and
+//    column, AI = 16 flop/B, above the ridge (5.7).
+//  * Everything is computed transposed so that "column of q" sits on the M index of every fragment and
+//    the C fragment of one product is, register for register, the A fragment of the next (the zero-
+//    shuffle fragment chaining of bt_wy.cuh): W^T = q^T V, U^T = W^T (-T)^T, q^T += U^T V^T.
+//    Lane (gq, r) = (lane / 4, lane % 4) holds rows 4r .. 4r+3 of column gq of a 16-row group (32
+//    contiguous bytes; the four lanes of a column cover one 128-byte line).
+//  * V tiles (16 rows x 64 reflectors of block P and of block P-1) are staged by the warps in turn
+//    with 16-byte cp.async (zero fill beyond N / Nv) into an 8-stage shared-memory ring
+//    [reflector][18 doubles]: the row stride 18 makes both B-fragment access patterns (LDS.128)
+//    bank-conflict free.  Completion on mbarriers, no CTA barrier in the loop.
+//  * A warp owns 1 or 2 slabs of 8 columns for ALL passes: W and U (2 x 16 doubles per slab) live in
+//    registers, q rows are loaded one group ahead.  CTAs never communicate; a CTA walks its slabs in
+//    rounds of up to 16.
+// Wasted tensor work: only the zero upper triangle of the first 64 rows of each block (0.2 % at
+// N = 32768) and the 64 x 64 T product per pass.
+#pragma once
+#include "bt_common.cuh"
+#include "bt_wy.cuh"        // dmma884, cp_async_mbar_arrive_noinc_wy
+
+namespace elpa2bt {
+
+struct B2fCfg {
+    static constexpr int NB = 64;                     // reflectors per block
+    static constexpr int GR = 16;                     // rows per group (one ring stage)
+    static constexpr int S = 18;                      // smem row stride per reflector (doubles): S/2 odd
+    static constexpr int PANEL = NB * S;              // doubles per panel tile
+    static constexpr int STAGE_DOUBLES = 2 * PANEL;   // panel 0: block P (update), panel 1: block P-1 (dot)
+    static constexpr int NS = 8, LGNS = 3, LAG = 4;
+    static constexpr int NW = 8;                      // warps per CTA
+    static constexpr int NGMAX = 2;                   // slabs per warp
+    static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
+    static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
+};
+
+struct B2fArgs {
+    int64_t N, nev, ldq, ldv, Nv;
+    int nbw;
+    const double *hv;      // N x Nv column-major, ldv
+    const double *tneg;    // npb x 64 x 64, row-major: tneg[p][i][k] = -T_p[i][k]
+    double *q;
+    int align16;           // q base and ldq*8 are 16-byte aligned
+};
+
+__host__ __device__ __forceinline__ int64_t b2f_nblocks(int64_t Nv) { return (Nv + B2fCfg::NB - 1) / B2fCfg::NB; }
+
+// ---- prepass: -T_p of every block (plain FP64; 0.1 % of the work of a call) -----------------------------
+// One CTA (256 threads) per block p.  S = V^T V over rows i0 .. N-1 (thread (ty, tx) owns the 4 x 4
+// sub-block S[4ty.., 4tx..]; V staged 16 rows at a time), then the larft recurrence column by column.
+__global__ void __launch_bounds__(256) b2f_tfactor_kernel(int64_t N, int64_t Nv, int nbw, const double *__restrict__ hv,
+                                                          int64_t ldv, const double *__restrict__ tau,
+                                                          double *__restrict__ tneg)
+{
+    constexpr int NB = B2fCfg::NB, RC = 16, SV = NB + 1;
+    __shared__ double Vs[RC * SV];                    // Vs[row][refl]
+    __shared__ double Sm[NB * SV];                    // Gram matrix, then T
+    __shared__ double taus[NB];
+    const int tid = threadIdx.x;
+    const int64_t p = blockIdx.x;
+    const int64_t j0 = p * NB;
+    const int nb = (int)((Nv - j0 < NB) ? Nv - j0 : NB);
+    const int64_t i0 = j0 + nbw;
+    const int ty = tid >> 4, tx = tid & 15;
+    double acc[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) acc[a][b] = 0.0;
+    if (tid < NB) taus[tid] = (tid < nb) ? tau[j0 + tid] : 0.0;
+    for (int64_t rb = i0; rb < N; rb += RC) {
+        // rows rb .. rb+15, lanes along rows (contiguous in hv)
+        for (int idx = tid; idx < RC * NB; idx += 256) {
+            const int c = idx >> 4, rr = idx & 15;
+            const int64_t row = rb + rr;
+            Vs[rr * SV + c] = (c < nb && row < N) ? hv[row + (j0 + c) * ldv] : 0.0;
+        }
+        __syncthreads();
+#pragma unroll 4
+        for (int rr = 0; rr < RC; ++rr) {
+            double a4[4], b4[4];
+#pragma unroll
+            for (int a = 0; a < 4; ++a) a4[a] = Vs[rr * SV + 4 * ty + a];
+#pragma unroll
+            for (int b = 0; b < 4; ++b) b4[b] = Vs[rr * SV + 4 * tx + b];
+#pragma unroll
+            for (int a = 0; a < 4; ++a)
+#pragma unroll
+                for (int b = 0; b < 4; ++b) acc[a][b] = fma(a4[a], b4[b], acc[a][b]);
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int a = 0; a < 4; ++a)
+#pragma unroll
+        for (int b = 0; b < 4; ++b) Sm[(4 * ty + a) * SV + 4 * tx + b] = acc[a][b];
+    __syncthreads();
+    // larft (forward, columnwise), in place: column i of T overwrites column i of S above the diagonal;
+    // thread r < i owns T[r][i] = -tau_i sum_{k = r}^{i-1} T[r][k] S[k][i]  (T[r][k], k < i, already final)
+    __shared__ double colS[NB];
+    for (int i = 0; i < NB; ++i) {
+        if (tid < i) colS[tid] = Sm[tid * SV + i];
+        __syncthreads();
+        if (tid < i) {
+            double s = 0.0;
+            for (int k = tid; k < i; ++k) s = fma((k == tid) ? taus[tid] : Sm[tid * SV + k], colS[k], s);
+            Sm[tid * SV + i] = -taus[i] * s;
+        }
+        __syncthreads();
+    }
+    // -T, row-major 64 x 64, zeros below the diagonal
+    double *out = tneg + p * (NB * NB);
+    for (int idx = tid; idx < NB * NB; idx += 256) {
+        const int i = idx >> 6, k = idx & 63;
+        out[idx] = (k > i) ? -Sm[i * SV + k] : (k == i ? -taus[i] : 0.0);
+    }
+}
+
+// ---- the sequence of ring items: pass P = npb .. 0, groups g = g_lo(P) .. g_hi ---------------------------
+// pass P updates with block P (P < npb; rows >= i0(P)) and accumulates the dot product of block P-1
+// (P >= 1; rows >= i0(P-1) = i0(P) - 64).  i0(p) = 64 p + nbw is a multiple of 16.
+struct B2fCursor {
+    int64_t P, g;
+};
+__device__ __forceinline__ int64_t b2f_glo(int64_t P, int nbw)
+{
+    const int64_t pb = P >= 1 ? P - 1 : 0;
+    return (pb * B2fCfg::NB + nbw) >> 4;
+}
+
+// stage one item (whole warp): panel 0 = V_P rows of group g (if the group is inside block P),
+// panel 1 = V_{P-1}.  1024 chunks of 16 bytes; lanes run along the 8 chunks of a reflector's 128 bytes.
+__device__ __forceinline__ void b2f_stage(const B2fArgs &a, double *stage, uint32_t bar_full, int64_t P, int64_t g,
+                                          int64_t npb, int lane)
+{
+    constexpr int NB = B2fCfg::NB, S = B2fCfg::S;
+    const int64_t row0 = g << 4;
+#pragma unroll
+    for (int panel = 0; panel < 2; ++panel) {
+        const int64_t blk = P - panel;
+        const bool on = (panel == 0) ? (P < npb && row0 >= P * NB + a.nbw) : (P >= 1);
+        if (!on) continue;                            // warp-uniform
+        const int ch = lane & 7;
+        const int64_t row = row0 + 2 * ch;
+        const uint32_t nbytes = (row + 1 < a.N) ? 16u : (row < a.N ? 8u : 0u);
+#pragma unroll 4
+        for (int t = 0; t < NB / 4; ++t) {
+            const int refl = 4 * t + (lane >> 3);
+            const int64_t j = blk * NB + refl;
+            const bool ok = (j < a.Nv) && nbytes;
+            const double *src = ok ? a.hv + row + j * a.ldv : a.hv;
+            cp_async16(smem_u32(stage + panel * B2fCfg::PANEL + refl * S + 2 * ch), src, ok ? nbytes : 0u);
+        }
+    }
+    cp_async_mbar_arrive_noinc_wy(bar_full);
+}
+
+// q rows 16 g + 4 r .. + 3 of this lane's column
+__device__ __forceinline__ void b2f_load4(const B2fArgs &a, const double *colp, bool colok, int64_t row, bool fast,
+                                          double (&y)[4])
+{
+    if (fast) {
+        const double2 u = *reinterpret_cast<const double2 *>(colp + row);
+        const double2 w = *reinterpret_cast<const double2 *>(colp + row + 2);
+        y[0] = u.x, y[1] = u.y, y[2] = w.x, y[3] = w.y;
+        return;
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e) y[e] = (colok && row + e < a.N) ? colp[row + e] : 0.0;
+}
+__device__ __forceinline__ void b2f_store4(const B2fArgs &a, double *colp, bool colok, int64_t row, bool fast,
+                                           const double (&y)[4])
+{
+    if (fast) {
+        *reinterpret_cast<double2 *>(colp + row) = make_double2(y[0], y[1]);
+        *reinterpret_cast<double2 *>(colp + row + 2) = make_double2(y[2], y[3]);
+        return;
+    }
+#pragma unroll
+    for (int e = 0; e < 4; ++e)
+        if (colok && row + e < a.N) colp[row + e] = y[e];
+}
+
+// ---- a warp with NG slabs of 8 columns, all passes ---------------------------------------------------------
+template <int NG>
+__device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *smem, const int lane, const int member,
+                                            const int nmem, const int64_t col0, uint32_t &it, int &duty)
+{
+    using C = B2fCfg;
+    constexpr int NB = C::NB, S = C::S, NSP = C::NS, LAG = C::LAG;
+    double *ring = reinterpret_cast<double *>(smem);
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + C::NS * 8;
+    const int gq = lane >> 2, r = lane & 3;
+    const int64_t N = a.N;
+    const int64_t npb = b2f_nblocks(a.Nv);
+    const int64_t ghi = (N - 1) >> 4;
+
+    double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq;
+    const int64_t ldq8 = a.ldq << 3;
+    const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
+    const bool allcols = a.align16 && (col0 + 8 * NG <= a.nev);
+
+    // staging cursor: item it + NSP - LAG of the sequence (every warp of the CTA keeps its own copy)
+    B2fCursor pc = {npb, b2f_glo(npb, a.nbw)};
+    auto advance = [&]() {
+        if (pc.P < 0) return;
+        if (pc.g < ghi) {
+            ++pc.g;
+        } else {
+            --pc.P;
+            pc.g = b2f_glo(pc.P, a.nbw);
+        }
+    };
+    auto stage_cursor = [&](uint32_t st) {
+        b2f_stage(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pc.P, pc.g, npb, lane);
+    };
+    // prologue of this round: items 0 .. NSP-LAG-1 (the ring is drained between rounds, see the kernel)
+    for (int i = 0; i < NSP - LAG; ++i) {
+        const uint32_t seq = it + i;
+        if (duty == member && pc.P >= 0) {
+            const uint32_t st = seq & (NSP - 1);
+            if (seq >= (uint32_t)NSP) mbar_wait(bar_empty + 8 * st, ((seq - NSP) >> C::LGNS) & 1);
+            stage_cursor(st);
+        }
+        advance();
+        duty = (duty + 1 == nmem) ? 0 : duty + 1;
+    }
+
+    double W[NG][8][2], U[NG][8][2], YA[NG][4], YB[NG][4];
+#pragma unroll
+    for (int s = 0; s < NG; ++s)
+#pragma unroll
+        for (int i = 0; i < 8; ++i) W[s][i][0] = W[s][i][1] = U[s][i][0] = U[s][i][1] = 0.0;
+
+    auto load_group = [&](int64_t g, double (&T)[NG][4]) {
+        const int64_t row = (g << 4) + 4 * r;
+        const bool fast = allcols && (row + 3 < N);
+#pragma unroll
+        for (int s = 0; s < NG; ++s) b2f_load4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, T[s]);
+    };
+
+    // one item (pass P, group g): Y = its rows of q on entry; Yn receives the next item's rows (loaded
+    // one item ahead into the other buffer, so no register copy ever waits for the load)
+    auto do_item = [&](const int64_t P, const int64_t g, double (&Y)[NG][4], double (&Yn)[NG][4]) {
+        // --- staging duty (rotates over the warps of the CTA, bt_wy.cuh)
+        {
+            const uint32_t seq = it + NSP - LAG;
+            if (duty == member && pc.P >= 0) {
+                const uint32_t st = seq & (NSP - 1);
+                if (seq >= (uint32_t)NSP) mbar_wait(bar_empty + 8 * st, ((seq - NSP) >> C::LGNS) & 1);
+                stage_cursor(st);
+            }
+            advance();
+            duty = (duty + 1 == nmem) ? 0 : duty + 1;
+        }
+        // --- prefetch the next item's rows of q (if an earlier pass touched them, this same lane wrote them)
+        {
+            int64_t gn = g + 1, Pn = P;
+            if (gn > ghi) {
+                Pn = P - 1;
+                gn = b2f_glo(Pn, a.nbw);
+            }
+            if (Pn >= 0) load_group(gn, Yn);
+        }
+        const uint32_t st = it & (NSP - 1), ph = (it >> C::LGNS) & 1;
+        mbar_wait(bar_full + 8 * st, ph);
+        const double *pa = ring + st * C::STAGE_DOUBLES;      // V_P tile
+        const double *pb = pa + C::PANEL;                     // V_{P-1} tile
+        const bool has_upd = (P < npb) && ((g << 4) >= P * NB + a.nbw);   // warp-uniform
+        const bool has_dot = P >= 1;
+
+        if (has_upd) {
+            // --- q^T += U^T V_P^T: K = 64 reflectors, chunk (i, e): k-slot r = reflector 8i + 2r + e;
+            //     n-tile 0 = rows 2n (C = Y[0], Y[2]), n-tile 1 = rows 2n + 1 (C = Y[1], Y[3])
+            const double *bp = pa + (2 * r) * S + 2 * gq;
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double2 b = *reinterpret_cast<const double2 *>(bp + (8 * i + e) * S);
+#pragma unroll
+                    for (int s = 0; s < NG; ++s) {
+                        dmma884(Y[s][0], Y[s][2], U[s][i][e], b.x, Y[s][0], Y[s][2]);
+                        dmma884(Y[s][1], Y[s][3], U[s][i][e], b.y, Y[s][1], Y[s][3]);
+                    }
+                }
+        }
+        if (has_dot) {
+            // --- W^T += q^T V_{P-1}: K = 16 rows, chunk e: k-slot r = row 4r + e; n-tile i = reflectors 8i + n.
+            //     Two n-tiles at a time: 2 NG independent accumulators in rotation
+            const double *bp = pb + gq * S + 4 * r;
+#pragma unroll
+            for (int i = 0; i < 8; i += 2) {
+                const double2 b00 = *reinterpret_cast<const double2 *>(bp + 8 * i * S);
+                const double2 b01 = *reinterpret_cast<const double2 *>(bp + 8 * i * S + 2);
+                const double2 b10 = *reinterpret_cast<const double2 *>(bp + 8 * (i + 1) * S);
+                const double2 b11 = *reinterpret_cast<const double2 *>(bp + 8 * (i + 1) * S + 2);
+                const double bv[2][4] = {{b00.x, b00.y, b01.x, b01.y}, {b10.x, b10.y, b11.x, b11.y}};
+#pragma unroll
+                for (int e = 0; e < 4; ++e)
+#pragma unroll
+                    for (int d = 0; d < 2; ++d)
+#pragma unroll
+                        for (int s = 0; s < NG; ++s)
+                            dmma884(W[s][i + d][0], W[s][i + d][1], Y[s][e], bv[d][e], W[s][i + d][0], W[s][i + d][1]);
+            }
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar_empty + 8 * st);
+        if (has_upd) {
+            const int64_t row = (g << 4) + 4 * r;
+            const bool fast = allcols && (row + 3 < N);
+#pragma unroll
+            for (int s = 0; s < NG; ++s) b2f_store4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, Y[s]);
+        }
+        ++it;
+        if (has_dot && g == ghi) {
+            // --- end of pass: U^T = W^T (-T_{P-1})^T.  n-tile i' = reflectors 8i' + n, k chunk (i, e): k-slot r =
+            //     reflector 8i + 2r + e; B[k][n] = -T[8i' + n][k], zero for k-tiles i < i' (T upper triangular)
+            const double *tp = a.tneg + (P - 1) * (NB * NB) + gq * NB + 2 * r;
+#pragma unroll
+            for (int ip = 0; ip < 8; ++ip) {
+                double c0[NG], c1[NG];
+#pragma unroll
+                for (int s = 0; s < NG; ++s) c0[s] = c1[s] = 0.0;
+#pragma unroll
+                for (int i = ip; i < 8; ++i) {
+                    const double2 b = __ldg(reinterpret_cast<const double2 *>(tp + 8 * ip * NB + 8 * i));
+#pragma unroll
+                    for (int s = 0; s < NG; ++s) {
+                        dmma884(c0[s], c1[s], W[s][i][0], b.x, c0[s], c1[s]);
+                        dmma884(c0[s], c1[s], W[s][i][1], b.y, c0[s], c1[s]);
+                    }
+                }
+#pragma unroll
+                for (int s = 0; s < NG; ++s) {
+                    U[s][ip][0] = c0[s];
+                    U[s][ip][1] = c1[s];
+                }
+            }
+#pragma unroll
+            for (int s = 0; s < NG; ++s)
+#pragma unroll
+                for (int i = 0; i < 8; ++i) W[s][i][0] = W[s][i][1] = 0.0;
+        }
+    };
+
+    // the item sequence, two items per trip so that the q buffers alternate
+    int64_t P = npb, g = b2f_glo(npb, a.nbw);
+    auto next = [&]() {
+        if (g < ghi) {
+            ++g;
+        } else {
+            --P;
+            g = b2f_glo(P, a.nbw);
+        }
+    };
+    load_group(g, YA);
+    while (P >= 0) {
+        do_item(P, g, YA, YB);
+        next();
+        if (P < 0) break;
+        do_item(P, g, YB, YA);
+        next();
+    }
+}
+
+// ---- the kernel ----------------------------------------------------------------------------------------------
+// grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid) and walks them in rounds of up to NW*NGMAX = 16;
+// in a round warp w takes n/8 slabs, +1 for the first n%8 warps (warps w and w+4 share a sub-partition).
+// All warps of the CTA traverse the same item sequence per round (also warps without a slab: they keep
+// the ring's duty rotation and empty-barrier counts simple), so a round is one full sequence of passes.
+__global__ void __launch_bounds__(256, 1) bt_b2f_kernel(const B2fArgs a)
+{
+    using C = B2fCfg;
+    extern __shared__ __align__(128) unsigned char smem[];
+    const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
+    const uint32_t bar_empty = bar_full + C::NS * 8;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int64_t nslab = (a.nev + 7) >> 3;
+    const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
+    const int64_t nmine = nslab * (blockIdx.x + 1) / gridDim.x - slab0;
+
+    int64_t done = 0;
+    while (done < nmine) {
+        int64_t nround = nmine - done;
+        if (nround > C::NW * C::NGMAX) nround = C::NW * C::NGMAX;
+        const int nact = (int)(nround < C::NW ? nround : C::NW);           // warps with work = ring members
+        if (threadIdx.x == 0) {
+            for (int i = 0; i < C::NS; ++i) {
+                if (done > 0) {
+                    mbar_inval(bar_full + 8 * i);
+                    mbar_inval(bar_empty + 8 * i);
+                }
+                mbar_init(bar_full + 8 * i, 32);                           // 32 cp.async arrivals (one per lane)
+                mbar_init(bar_empty + 8 * i, (uint32_t)nact);
+            }
+            mbar_fence_init();
+        }
+        __syncthreads();
+        uint32_t it = 0;
+        int duty = 0;
+        const int base = (int)(nround / C::NW), extra = (int)(nround % C::NW);
+        const int ng = base + (warp < extra ? 1 : 0);
+        const int64_t wslab0 = slab0 + done + (int64_t)warp * base + (warp < extra ? warp : extra);
+        if (ng == 2)
+            b2f_consume<2>(a, smem, lane, warp, nact, wslab0 << 3, it, duty);
+        else if (ng == 1)
+            b2f_consume<1>(a, smem, lane, warp, nact, wslab0 << 3, it, duty);
+        done += nround;
+        __syncthreads();                                                   // ring drained before it is re-initialised
+    }
+}
+
+inline size_t b2f_scratch_bytes(int64_t N, int nbw)
+{
+    const int64_t Nv = (N - nbw - 1 > 0) ? N - nbw - 1 : 0;
+    return (size_t)b2f_nblocks(Nv) * B2fCfg::NB * B2fCfg::NB * sizeof(double);
+}
+
+// launch plan: persistent grid, one CTA per SM, rounds of 16 slabs
+inline int64_t b2f_grid(int64_t nev, int nsm)
+{
+    const int64_t nslab = (nev + 7) >> 3;
+    return nslab < nsm ? nslab : nsm;
+}
+
+inline cudaError_t launch_b2f(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv, const double *tau, double *q,
+                              int64_t ldq, int align16, int nsm, void *scratch, cudaStream_t st)
+{
+    const int64_t Nv = N - nbw - 1;
+    const int64_t npb = b2f_nblocks(Nv);
+    double *tneg = (double *)scratch;
+    b2f_tfactor_kernel<<<(unsigned)npb, 256, 0, st>>>(N, Nv, nbw, hv, ldv, tau, tneg);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if ((e = set_max_smem((const void *)bt_b2f_kernel, B2fCfg::SMEM_BYTES)) != cudaSuccess) return e;
+    B2fArgs a;
+    a.N = N;
+    a.nev = nev;
+    a.ldq = ldq;
+    a.ldv = ldv;
+    a.Nv = Nv;
+    a.nbw = nbw;
+    a.hv = hv;
+    a.tneg = tneg;
+    a.q = q;
+    a.align16 = align16;
+    bt_b2f_kernel<<<(unsigned)b2f_grid(nev, nsm), 256, B2fCfg::SMEM_BYTES, st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace elpa2bt

@@ -16,6 +16,7 @@
 #include "bt_wy.cuh"
 #include "bt_wyz.cuh"
 #include "bc_chase.cuh"
+#include "bt_b2f.cuh"
 
 using namespace elpa2bt;
 
@@ -348,6 +349,34 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, 
     }
     if (err != cudaSuccess) return (int)err;
     g_last_launches = (int)(nl > 0x7fffffff ? 0x7fffffff : nl);
+    return 0;
+}
+
+int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv, const double *tau,
+                                  double *q, int64_t ldq, void *stream)
+{
+    if (N < 0) return -1;
+    if (nbw < 16 || (nbw & 15) != 0) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (N - nbw - 1 <= 0 || nev == 0) return 0;          // no reflector: P = I
+    if (!hv || ((uintptr_t)hv & 15) != 0) return -4;
+    if (ldv < N || (ldv & 1) != 0) return -5;
+    if (!tau || ((uintptr_t)tau & 7) != 0) return -6;
+    if (!q || ((uintptr_t)q & 7) != 0) return -7;
+    if (ldq < N) return -8;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    cudaMemPool_t pool = scratch_pool(&e);
+    if (!pool) return (int)e;
+    void *scratch = nullptr;
+    if ((e = cudaMallocFromPoolAsync(&scratch, b2f_scratch_bytes(N, nbw), pool, st)) != cudaSuccess) return (int)e;
+    const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
+    e = launch_b2f(N, nbw, nev, hv, ldv, tau, q, ldq, align16, sm_count(), scratch, st);
+    const cudaError_t e2 = cudaFreeAsync(scratch, st);
+    if (e != cudaSuccess) return (int)e;
+    if (e2 != cudaSuccess) return (int)e2;
+    g_last_launches = 2;
     return 0;
 }
 

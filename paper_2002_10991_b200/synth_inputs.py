@@ -165,3 +165,45 @@ def synthetic_reflectors(lengths, nbw: int, seed: int, cplx: bool = False, devic
         tau = 2.0 / nrm2
     tau = torch.where(L > 1, tau, torch.zeros_like(tau))
     return v.contiguous(), tau.contiguous()
+
+
+def synthetic_full_reflectors(N: int, nbw: int, seed: int, cplx: bool = False, device: str = "cpu", ldv=None):
+    """Unitary synthetic reflector set in the layout of the band -> full back-transformation (Eq. 6e;
+    include/elpa2_bt.h): returns torch tensors (hv, tau) with hv of shape (N, Nv) stored column-major
+    (the transposed view of a (Nv, ldv) tensor), Nv = max(N - nbw - 1, 0).  Column j: zeros in rows
+    < j + nbw, 1 at row j + nbw, uniform entries scaled by 1.3 / sqrt(L) below (L = N - nbw - j: the range
+    a QR of a random panel gives); tau = 2 / ||v||^2 (real) or (1 + e^{i theta}) / ||v||^2 (complex), so that
+    every H = I - tau v v^H is unitary up to rounding.  Stands in for the output of a full -> band
+    reduction at sizes where the oracle's O(N^3) reduction is out of reach."""
+    import torch
+
+    Nv = max(N - nbw - 1, 0)
+    ldv = ldv or (N + (N & 1))
+    dt = torch.complex128 if cplx else torch.float64
+    back = torch.zeros((max(Nv, 1), ldv), dtype=dt, device=device)
+    tau = torch.zeros((Nv,), dtype=dt, device=device)
+    gen = torch.Generator(device=device)
+    gen.manual_seed(seed)
+    rows = torch.arange(N, device=device)[None, :]
+    step = 1024
+    for j0 in range(0, Nv, step):
+        j1 = min(j0 + step, Nv)
+        head = (torch.arange(j0, j1, device=device) + nbw)[:, None]
+        L = (N - head).to(torch.float64)
+        shape = (j1 - j0, N, 2) if cplx else (j1 - j0, N)
+        v = torch.rand(shape, generator=gen, device=device, dtype=torch.float64) * 2.0 - 1.0
+        scale = 1.3 / torch.sqrt(L)
+        if cplx:
+            v = torch.view_as_complex((v * scale[:, :, None]).contiguous())
+        else:
+            v = v * scale
+        v = torch.where(rows > head, v, torch.zeros_like(v))
+        v = torch.where(rows == head, torch.ones_like(v), v)
+        nrm2 = (v.real ** 2 + v.imag ** 2).sum(dim=1) if cplx else (v * v).sum(dim=1)
+        if cplx:
+            theta = (torch.rand(j1 - j0, generator=gen, device=device, dtype=torch.float64) - 0.5) * 1.5
+            tau[j0:j1] = (1.0 + torch.polar(torch.ones_like(theta), theta)) / nrm2
+        else:
+            tau[j0:j1] = 2.0 / nrm2
+        back[j0:j1, :N] = v
+    return back[:Nv].t()[:N, :], tau
