@@ -50,8 +50,36 @@ CONFIGS = {
 METRIC = "back-transform FP64 GFLOP/s (2N^2*nev real / 8N^2*nev cplx)"
 # FP64 ALU roofline: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from profiles/ (ncu --set full), by config
-NCU_TRAFFIC_BYTES = {4: 2.603878e12 + 2.202669e12}    # profiles/r1_c_wy_config4.md
+
+
+def source_sha() -> str:
+    """Fingerprint of the CUDA sources the loaded library was built from (the .git directory does not
+    travel to the GPU box, so a commit hash is not available there): sha256 over csrc/*, 16 hex digits."""
+    import hashlib
+
+    d = os.path.join(ROOT, "paper_2002_10991_b200", "csrc")
+    h = hashlib.sha256()
+    for f in sorted(os.listdir(d)):
+        if f.endswith((".cu", ".cuh")):
+            h.update(f.encode())
+            h.update(open(os.path.join(d, f), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def lookup_traffic(step: str, workload: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from
+    profiles/traffic.json (written from an ``ncu --set full`` capture; each entry names its profile and
+    the source fingerprint it was taken at).  None unless an entry matches this step, this workload AND
+    the sources the library in use was built from: a number measured on other code is not reported."""
+    try:
+        entries = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))["entries"]
+    except (OSError, ValueError, KeyError):
+        return None, None
+    sha = source_sha()
+    for e in entries:
+        if e.get("step") == step and e.get("workload") == workload and e.get("source_sha") == sha:
+            return float(e["dram_bytes_per_launch"]), e.get("profile")
+    return None, None
 
 
 def model_flops(cplx: bool, N: int, nev: int) -> float:
@@ -199,9 +227,10 @@ def chase_kernel_name(cplx: bool, nbw: int) -> str:
 
 
 def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
-    """--chase: SURVEY.md 8(f) NEXT-1, first version.  One step = one band -> tridiagonal reduction of the
-    config's seeded band matrix on the device (about 3N wavefront launches); model work 6 N^2 nbw flops
-    (SURVEY O3).  Replicas only: the chase does not shard."""
+    """--chase: SURVEY.md 8(f) NEXT-1.  One step = one band -> tridiagonal reduction of the config's seeded
+    band matrix on the device (one persistent cooperative kernel + the d/e extraction; one launch per
+    wavefront only with ELPA2_BC_WAVEFRONT=1); model work 6 N^2 nbw flops.  Replicas only: the
+    chase does not shard."""
     import numpy as np
     import torch
 
@@ -258,6 +287,190 @@ def run_chase(args, N, nbw, cplx, seed, rank, world, local_rank) -> None:
         }), flush=True)
 
 
+METRIC_6E = "band->full back-transform FP64 GFLOP/s (4*nev*sum(L) real / 16*nev*sum(L) cplx)"
+
+
+def b2f_flops(cplx: bool, N: int, nbw: int, nev: int) -> float:
+    """Algorithmic flops of Eq. 6e: one reflector of length L on one column = 4 L flops (16 L complex);
+    sum over j < Nv of L_j = N - nbw - j is Nv (Nv + 3) / 2."""
+    Nv = max(N - nbw - 1, 0)
+    return (16.0 if cplx else 4.0) * nev * (Nv * (Nv + 3) / 2.0)
+
+
+def b2f_workload_name(cfg: int) -> str:
+    cplx, N, nbw, nev, _, _ = CONFIGS[cfg]
+    tag = "custom (--shape)" if cfg == 0 else f"6e-config{cfg}"
+    return f"{tag}: {'complex' if cplx else 'real'} FP64 N={N} nbw={nbw} nev={nev}"
+
+
+def b2f_oracle_cols(cplx: bool, N: int, nbw: int, cores: int) -> int:
+    per_col = b2f_flops(cplx, N, nbw, 1) / (2.9e9 if cplx else 1.9e9)
+    return cores * max(1, min(64, int(16.0 / max(per_col, 1e-9))))
+
+
+def b2f_oracle_run(cplx, N, nbw, hv_np, tau_np, ncols, seed):
+    import numpy as np
+
+    import oracle
+
+    rng = np.random.default_rng(seed)
+    x = rng.standard_normal((N, ncols))
+    if cplx:
+        x = x + 1j * rng.standard_normal((N, ncols))
+    x = np.asfortranarray(x)
+    t0 = time.perf_counter()
+    oracle.band_to_full_back(N, nbw, hv_np, tau_np, x)
+    return time.perf_counter() - t0, oracle.num_threads()
+
+
+def run_b2f_reference(args, rank: int) -> None:
+    """--impl reference --step 6e: the oracle's plain sequential application on a column sample."""
+    if rank != 0:
+        return
+    import oracle
+    from paper_2002_10991_b200 import synth_inputs as si
+
+    cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
+    cores = oracle.num_threads()
+    hv, tau = si.synthetic_full_reflectors(N, nbw, seed_r, cplx, "cpu")
+    hv_np, tau_np = hv.numpy(), tau.numpy()
+    ncols = b2f_oracle_cols(cplx, N, nbw, cores)
+    times = []
+    for i in range(args.warmup + args.steps):
+        t, _ = b2f_oracle_run(cplx, N, nbw, hv_np, tau_np, ncols, seed_x + i)
+        if i >= args.warmup:
+            times.append(t)
+    total = sum(times)
+    gflops = b2f_flops(cplx, N, nbw, ncols) * len(times) / total / 1e9
+    sample = f"{ncols} seeded N(0,1) columns of {nev} per step (columns are independent, PAPER.md:134)"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC_6E, "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": b2f_workload_name(args.config), "reflectors": "synthetic unitary set (host-generated)"},
+        "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
+        "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }), flush=True)
+
+
+def run_b2f(args, rank, world, local_rank, dist) -> None:
+    """--step 6e: SURVEY.md 8(f) NEXT-2.  One step = one call of ``elpa2_trans_ev_band_to_full_d`` over the
+    whole N x nev block (T-factor prepass + the fused DMMA kernel).  Reflectors: the seeded synthetic
+    unitary set in the Eq. 6e layout (the oracle's O(N^3) full -> band reduction is out of reach at these
+    sizes); q i.i.d. N(0,1); both generated on the device.  N > 1: column shards, no collective."""
+    import torch
+
+    from paper_2002_10991_b200 import binding, shard, synth_inputs as si
+
+    cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
+    if cplx:
+        raise SystemExit("--step 6e: the complex path is not built yet")
+    esz = 16 if cplx else 8
+    Nv = max(N - nbw - 1, 0)
+    flops = b2f_flops(cplx, N, nbw, nev)
+    hv, tau = si.synthetic_full_reflectors(N, nbw, seed_r, cplx, "cuda")
+    q = si.gaussian_block(N, nev, seed_x + 7919 * rank, cplx, "cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        binding.trans_ev_band_to_full(N, nbw, hv, tau, q, stream=stream)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dfma_tf = binding.probe_fp64(0, 8192, 20)
+    dmma_tf = binding.probe_fp64(1, 8192, 20)
+    ncheck = min(nev, 64)
+    nrm0 = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    launches = 0
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        ev[0].record(stream)
+        for i in range(args.steps):
+            step()
+            launches += binding.last_launch_count()
+            ev[i + 1].record(stream)
+        barrier()
+    clk = clocks.summary()
+    step_ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    total_ms = shard.max_over_ranks(ev[0].elapsed_time(ev[args.steps]), dist, "cuda")
+    ms_per_step = total_ms / args.steps
+    value = shard.aggregate_throughput(flops, world, ms_per_step * 1e-3) / 1e9
+    nrm = torch.linalg.vector_norm(q[:, :ncheck], dim=0)
+    norm_dev = float((nrm / nrm0 - 1.0).abs().max().item())
+
+    e2e = None
+    if args.e2e_steps > 0:
+        ldv = hv.stride(1) if Nv > 1 else N + (N & 1)
+        hv_h = torch.empty((Nv, ldv), dtype=hv.dtype, pin_memory=True)
+        hv_h[:, :N].copy_(hv.t())
+        if ldv > N:
+            hv_h[:, N:].zero_()
+        tau_h = torch.empty(tau.shape, dtype=tau.dtype, pin_memory=True).copy_(tau)
+        q_h = torch.empty((nev, N), dtype=q.dtype, pin_memory=True).copy_(q.t())
+        torch.cuda.synchronize()
+        hv_np, tau_np, q_np = hv_h.numpy().T, tau_h.numpy(), q_h.numpy().T
+        binding.trans_ev_band_to_full_host(N, nbw, hv_np, tau_np, q_np)         # warm-up: scratch alloc
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            binding.trans_ev_band_to_full_host(N, nbw, hv_np, tau_np, q_np)
+            launches += binding.last_launch_count()
+        torch.cuda.synchronize()
+        dt = shard.max_over_ranks(time.perf_counter() - t0, dist, "cuda")
+        e2e = {"value": world * flops * args.e2e_steps / dt / 1e9, "unit": "GFLOP/s",
+               "h2d_bytes_per_step": (ldv * Nv + Nv + N * nev) * esz, "d2h_bytes_per_step": N * nev * esz,
+               "steps": args.e2e_steps, "timer": "host wall clock around synchronous calls"}
+        del hv_h, tau_h, q_h
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        import oracle
+
+        cores = oracle.num_threads()
+        ncols = b2f_oracle_cols(cplx, N, nbw, cores)
+        hv_np = hv.t().cpu().numpy().T                       # (N, Nv), column-major, whatever ldv the copy keeps
+        tsec, cores = b2f_oracle_run(cplx, N, nbw, hv_np, tau.cpu().numpy(), ncols, seed_x)
+        cpu = {"value": b2f_flops(cplx, N, nbw, ncols) / tsec / 1e9, "unit": "GFLOP/s", "cores": cores,
+               "kind": "oracle", "seconds": tsec,
+               "sample": f"{ncols} seeded N(0,1) columns of {nev}, all {Nv} reflectors (columns are independent, PAPER.md:134)"}
+        del hv_np
+
+    if rank == 0:
+        kern_ms = sum(step_ms) / len(step_ms)
+        achieved = flops / (kern_ms * 1e-3) / 1e12
+        traffic, traffic_profile = lookup_traffic("6e", b2f_workload_name(args.config))
+        print(json.dumps({
+            "metric": METRIC_6E, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": b2f_workload_name(args.config), "N": N, "nbw": nbw, "nev_per_gpu": nev, "reflectors_Nv": Nv,
+                       "reflectors": "synthetic unitary set in the Eq. 6e layout, device-generated (DESIGN.md input recipe)",
+                       "l2": "inputs larger than L2 (%.2f GiB of q + reflectors per step)" % ((N * Nv + 2 * N * nev) * esz / 2**30),
+                       "parallelism": "column shards, no collective" if world > 1 else "single GPU",
+                       "source_sha": source_sha()},
+            "roofline": {"bound": "tensor", "achieved": achieved, "peak": dmma_tf, "unit": "TFLOP/s", "frac": achieved / dmma_tf,
+                         "peak_source": "FP64 DMMA m8n8k4 probe measured in this run (elpa2_bt_probe_fp64 kind 1); "
+                                        "MEASURED_PEAKS.json has no FP64 figure",
+                         "peak_dfma_probe": dfma_tf, "peak_dmma_probe": dmma_tf, "peak_nominal": NOMINAL_FP64_TFLOPS,
+                         "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                         "kernel": "bt_b2f_kernel (the interval also holds its T-factor prepass kernel)",
+                         "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
+                         "traffic": traffic, "traffic_profile": traffic_profile},
+            "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
+            "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},
+        }), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -271,6 +484,11 @@ def main() -> None:
                     help="library variant for A/B runs (include/elpa2_bt.h): 0 default, 2 register window, 3 two chains per pass")
     ap.add_argument("--chase", action="store_true",
                     help="time SURVEY 8(f) NEXT-1 instead: the GPU bulge chase (real configs) that produces the reflectors")
+    ap.add_argument("--step", default="6d", choices=["6d", "6e"],
+                    help="6d (default): tridiagonal -> band back-transformation, the north star; 6e: SURVEY 8(f) NEXT-2, "
+                         "band -> full back-transformation on the same config's N, nbw, nev (real configs)")
+    ap.add_argument("--nev-frac", type=float, default=None,
+                    help="partial spectrum (PAPER.md:218): replace nev by round(frac * N)")
     ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",
                     help="profiling aid: replace the chosen config's shape (named 'custom' in the output)")
     args = ap.parse_args()
@@ -282,12 +500,20 @@ def main() -> None:
         CONFIGS[0] = (t == "z", int(n_), int(b_), int(e_), 1000, 2000)
         args.config = 0
 
+    if args.nev_frac is not None:
+        c = CONFIGS[args.config]
+        CONFIGS[0] = (c[0], c[1], c[2], max(1, int(round(args.nev_frac * c[1]))), c[4], c[5])
+        args.config = 0
+
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
 
     if args.impl == "reference":
-        run_reference(args, rank)
+        if args.step == "6e":
+            run_b2f_reference(args, rank)
+        else:
+            run_reference(args, rank)
         return
 
     import numpy as np
@@ -309,6 +535,9 @@ def main() -> None:
     flops = model_flops(cplx, N, nev)
     if args.chase:
         run_chase(args, N, nbw, cplx, seed_r, rank, world, local_rank)
+        return
+    if args.step == "6e":
+        run_b2f(args, rank, world, local_rank, dist)
         return
 
     # ---- inputs, generated on the device (each rank: its own nev columns, same reflectors) ----
@@ -400,6 +629,7 @@ def main() -> None:
     if rank == 0:
         kern_ms = sum(step_ms) / len(step_ms)
         achieved = flops / (kern_ms * 1e-3) / 1e12
+        traffic, traffic_profile = lookup_traffic("6d", workload_name(args.config)) if args.variant == 0 else (None, None)
         out = {
             "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
@@ -411,7 +641,7 @@ def main() -> None:
                               % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
                              else "inputs smaller than L2; config is latency-bound (DESIGN.md)",
                        "parallelism": "column shards, no collective" if world > 1 else "single GPU",
-                       "variant": args.variant},
+                       "variant": args.variant, "source_sha": source_sha()},
             "roofline": {"bound": "tensor" if tensor_path else "alu", "achieved": achieved, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved / peak_tf,
                          "peak_source": ("FP64 %s probe measured in this run (elpa2_bt_probe_fp64 kind %d); "
@@ -422,7 +652,7 @@ def main() -> None:
                          "kernel": ("bt_wyz_kernel" if cplx else "bt_wy_kernel")
                                    + " (the interval also holds its T-factor prepass kernel)",
                          "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
-                         "traffic": NCU_TRAFFIC_BYTES.get(args.config)},
+                         "traffic": traffic, "traffic_profile": traffic_profile},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},
         }

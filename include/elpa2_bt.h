@@ -116,6 +116,13 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau,
 int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv,
                                   const double *tau, double *q, int64_t ldq, void *stream);
 
+/* Same operation with HOST buffers (pageable or pinned), synchronous: H2D of hv, tau and q, the two
+ * kernels, D2H of q (what bench.py --step 6e reports as e2e).  Device scratch cached as for
+ * elpa2_trans_ev_tridi_to_band_host.  Argument positions: is_complex=1, N=2, nbw=3, nev=4, hv=5, ldv=6,
+ * tau=7, q=8, ldq=9.  is_complex must be 0 (the complex path has the device entry point only). */
+int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hv,
+                                     int64_t ldv, const void *tau, void *q, int64_t ldq);
+
 /* Layout helpers (host, pure integer arithmetic; R3).  G = number of reflector slots. */
 /* Length L = min(nbw, N-1-s-k*nbw) of every slot in slot order (all but the last
  * reflector of a sweep have length nbw): writes min(G, cap) entries to `out` (HOST, may be NULL to

@@ -23,6 +23,7 @@ EXPORTS = (
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
     "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
     "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d",
+    "elpa2_trans_ev_band_to_full_host",
 )
 
 
@@ -57,6 +58,8 @@ def lib() -> ctypes.CDLL:
             getattr(L, nm).restype = i32
         L.elpa2_trans_ev_band_to_full_d.argtypes = [i64, i32, i64, vp, i64, vp, vp, i64, vp]
         L.elpa2_trans_ev_band_to_full_d.restype = i32
+        L.elpa2_trans_ev_band_to_full_host.argtypes = [i32, i64, i32, i64, vp, i64, vp, vp, i64]
+        L.elpa2_trans_ev_band_to_full_host.restype = i32
         L.elpa2_bt_release_scratch.argtypes = []
         L.elpa2_bt_release_scratch.restype = i32
         L.elpa2_bt_plan.argtypes = [i32, i64, i32, i64, i32, ctypes.POINTER(i64)]
@@ -216,6 +219,24 @@ def trans_ev_band_to_full(N: int, nbw: int, hv, tau, q, stream=None) -> None:
         raise ValueError("hv, tau and q must live on the current CUDA device")
     rc = lib().elpa2_trans_ev_band_to_full_d(N, nbw, nev, hv.data_ptr(), ldv, tau.data_ptr(), q.data_ptr(), ldq,
                                              _stream_ptr(stream))
+    if rc != 0:
+        raise Elpa2BtError(rc)
+
+
+def trans_ev_band_to_full_host(N: int, nbw: int, hv, tau, q) -> None:
+    """Eq. 6e with HOST numpy arrays: ``hv`` Fortran-ordered (ldv, Nv) block whose first N rows are the
+    reflectors (ldv = hv.shape[0] even), ``tau`` (Nv,), ``q`` Fortran-ordered (N, nev), updated in place."""
+    import numpy as np
+
+    if np.iscomplexobj(q) or q.dtype != np.float64 or hv.dtype != np.float64 or tau.dtype != np.float64:
+        raise ValueError("float64 throughout")
+    Nv = max(N - nbw - 1, 0)
+    if q.ndim != 2 or q.shape[0] != N or not q.flags.f_contiguous:
+        raise ValueError("q must be Fortran-contiguous (N, nev)")
+    if Nv > 0 and (hv.ndim != 2 or hv.shape[1] != Nv or hv.shape[0] < N or not hv.flags.f_contiguous):
+        raise ValueError("hv must be Fortran-contiguous (ldv >= N, Nv)")
+    rc = lib().elpa2_trans_ev_band_to_full_host(0, N, nbw, q.shape[1], hv.ctypes.data, hv.shape[0], tau.ctypes.data,
+                                                q.ctypes.data, max(N, 1))
     if rc != 0:
         raise Elpa2BtError(rc)
 

@@ -143,27 +143,39 @@ __device__ __forceinline__ int64_t b2f_glo(int64_t P, int nbw)
 }
 
 // stage one item (whole warp): panel 0 = V_P rows of group g (if the group is inside block P),
-// panel 1 = V_{P-1}.  1024 chunks of 16 bytes; lanes run along the 8 chunks of a reflector's 128 bytes.
+// panel 1 = V_{P-1}.  1024 chunks of 16 bytes; lanes run along the 8 chunks of a reflector's 128 bytes,
+// four reflectors per instruction.  Warp-uniform fast path (group inside the matrix, block full): one
+// cp.async and one pointer increment per chunk.
 __device__ __forceinline__ void b2f_stage(const B2fArgs &a, double *stage, uint32_t bar_full, int64_t P, int64_t g,
                                           int64_t npb, int lane)
 {
     constexpr int NB = B2fCfg::NB, S = B2fCfg::S;
     const int64_t row0 = g << 4;
+    const int ch = lane & 7, lr = lane >> 3;
+    const int64_t row = row0 + 2 * ch;
+    const bool rows_full = row0 + 16 <= a.N;          // warp-uniform
+    const int64_t ld4 = a.ldv << 2;
 #pragma unroll
     for (int panel = 0; panel < 2; ++panel) {
         const int64_t blk = P - panel;
         const bool on = (panel == 0) ? (P < npb && row0 >= P * NB + a.nbw) : (P >= 1);
         if (!on) continue;                            // warp-uniform
-        const int ch = lane & 7;
-        const int64_t row = row0 + 2 * ch;
-        const uint32_t nbytes = (row + 1 < a.N) ? 16u : (row < a.N ? 8u : 0u);
+        const double *src = a.hv + row + (blk * NB + lr) * a.ldv;
+        const uint32_t dst = smem_u32(stage + panel * B2fCfg::PANEL + lr * S + 2 * ch);
+        if (rows_full && (blk + 1) * NB <= a.Nv) {
+#pragma unroll
+            for (int t = 0; t < NB / 4; ++t) {
+                cp_async16(dst + t * (4 * S * 8), src, 16u);
+                src += ld4;
+            }
+        } else {
+            const uint32_t nbytes = (row + 1 < a.N) ? 16u : (row < a.N ? 8u : 0u);
 #pragma unroll 4
-        for (int t = 0; t < NB / 4; ++t) {
-            const int refl = 4 * t + (lane >> 3);
-            const int64_t j = blk * NB + refl;
-            const bool ok = (j < a.Nv) && nbytes;
-            const double *src = ok ? a.hv + row + j * a.ldv : a.hv;
-            cp_async16(smem_u32(stage + panel * B2fCfg::PANEL + refl * S + 2 * ch), src, ok ? nbytes : 0u);
+            for (int t = 0; t < NB / 4; ++t) {
+                const bool ok = (blk * NB + 4 * t + lr < a.Nv) && nbytes;
+                cp_async16(dst + t * (4 * S * 8), ok ? src : a.hv, ok ? nbytes : 0u);
+                src += ld4;
+            }
         }
     }
     cp_async_mbar_arrive_noinc_wy(bar_full);
@@ -249,7 +261,7 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
 
     auto load_group = [&](int64_t g, double (&T)[NG][4]) {
         const int64_t row = (g << 4) + 4 * r;
-        const bool fast = allcols && (row + 3 < N);
+        const bool fast = allcols && ((g << 4) + 16 <= N);        // warp-uniform
 #pragma unroll
         for (int s = 0; s < NG; ++s) b2f_load4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, T[s]);
     };
@@ -257,6 +269,14 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
     // one item (pass P, group g): Y = its rows of q on entry; Yn receives the next item's rows (loaded
     // one item ahead into the other buffer, so no register copy ever waits for the load)
     auto do_item = [&](const int64_t P, const int64_t g, double (&Y)[NG][4], double (&Yn)[NG][4]) {
+        // --- the rows of q that item it + NSP - LAG (the staging cursor) will read go to L2 now: q streams from
+        //     DRAM one 128-byte line per column and item, and a register load issued one item ahead does
+        //     not cover that latency (20 % of the issue slots stalled on it) -- an L2 hit it does
+        if (pc.P >= 0 && allcols) {
+            const double *pp = cb + (pc.g << 4) + 4 * r;
+#pragma unroll
+            for (int s = 0; s < NG; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + s * ldq8));
+        }
         // --- staging duty (rotates over the warps of the CTA, bt_wy.cuh)
         {
             const uint32_t seq = it + NSP - LAG;
@@ -267,15 +287,6 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
             }
             advance();
             duty = (duty + 1 == nmem) ? 0 : duty + 1;
-        }
-        // --- prefetch the next item's rows of q (if an earlier pass touched them, this same lane wrote them)
-        {
-            int64_t gn = g + 1, Pn = P;
-            if (gn > ghi) {
-                Pn = P - 1;
-                gn = b2f_glo(Pn, a.nbw);
-            }
-            if (Pn >= 0) load_group(gn, Yn);
         }
         const uint32_t st = it & (NSP - 1), ph = (it >> C::LGNS) & 1;
         mbar_wait(bar_full + 8 * st, ph);
@@ -300,6 +311,20 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
                     }
                 }
         }
+        // --- the next item's rows of q go into the other buffer (if an earlier pass touched them, this same
+        //     lane wrote them).  Issued HERE, after the first use of this item's rows: issued at the top of
+        //     the item, the loads shared a scoreboard with the loads of the item before, and the first
+        //     use of Y then waited for the loads just issued (a full L2/DRAM latency per item).
+        asm volatile("" ::: "memory");
+        {
+            int64_t gn = g + 1, Pn = P;
+            if (gn > ghi) {
+                Pn = P - 1;
+                gn = b2f_glo(Pn, a.nbw);
+            }
+            if (Pn >= 0) load_group(gn, Yn);
+        }
+        asm volatile("" ::: "memory");
         if (has_dot) {
             // --- W^T += q^T V_{P-1}: K = 16 rows, chunk e: k-slot r = row 4r + e; n-tile i = reflectors 8i + n.
             //     Two n-tiles at a time: 2 NG independent accumulators in rotation
@@ -324,7 +349,7 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
         if (lane == 0) mbar_arrive(bar_empty + 8 * st);
         if (has_upd) {
             const int64_t row = (g << 4) + 4 * r;
-            const bool fast = allcols && (row + 3 < N);
+            const bool fast = allcols && ((g << 4) + 16 <= N);    // warp-uniform
 #pragma unroll
             for (int s = 0; s < NG; ++s) b2f_store4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, Y[s]);
         }

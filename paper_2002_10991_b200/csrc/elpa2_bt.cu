@@ -380,6 +380,38 @@ int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double 
     return 0;
 }
 
+int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hv, int64_t ldv,
+                                     const void *tau, void *q, int64_t ldq)
+{
+    if (is_complex) return -1;                           // complex: device entry point only, for now
+    const size_t esz = 8;
+    if (N < 0) return -2;
+    if (nbw < 16 || (nbw & 15) != 0) return -3;
+    if (nev < 0) return -4;
+    const int64_t Nv = N - nbw - 1;
+    if (Nv <= 0 || nev == 0) { g_last_launches = 0; return 0; }
+    if (!hv) return -5;
+    if (ldv < N || (ldv & 1) != 0) return -6;
+    if (!tau) return -7;
+    if (!q) return -8;
+    if (ldq < N) return -9;
+    std::lock_guard<std::mutex> lock(g_mu);
+    const size_t bv = (size_t)ldv * Nv * esz, bt = (size_t)Nv * esz, bq = (size_t)ldq * nev * esz;
+    cudaError_t e;
+    if ((e = g_sv.reserve(bv)) != cudaSuccess) return (int)e;
+    if ((e = g_st.reserve(bt)) != cudaSuccess) return (int)e;
+    if ((e = g_sq.reserve(bq)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sv.p, hv, bv, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_st.p, tau, bt, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sq.p, q, bq, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    const int rc = elpa2_trans_ev_band_to_full_d(N, nbw, nev, (const double *)g_sv.p, ldv, (const double *)g_st.p,
+                                                 (double *)g_sq.p, ldq, 0);
+    if (rc != 0) return rc < 0 ? rc - 1 : rc;            // argument positions shift by one (is_complex)
+    if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
+    return 0;
+}
+
 int64_t elpa2_hh_count(int64_t N, int nbw)
 {
     const int lg = lg_of(nbw);
