@@ -21,12 +21,14 @@
 //    Lane (gq, r) = (lane / 4, lane % 4) holds rows 4r .. 4r+3 of column gq of a 16-row group (32
 //    contiguous bytes; the four lanes of a column cover one 128-byte line).
 //  * V tiles (16 rows x 64 reflectors of block P and of block P-1) are staged by the warps in turn
-//    with 16-byte cp.async (zero fill beyond N / Nv) into an 8-stage shared-memory ring
+//    with 16-byte cp.async (zero fill beyond N / Nv) into a 4-stage shared-memory ring
 //    [reflector][18 doubles]: the row stride 18 makes both B-fragment access patterns (LDS.128)
 //    bank-conflict free.  Completion on mbarriers, no CTA barrier in the loop.
 //  * A warp owns 1 or 2 slabs of 8 columns for ALL passes: W and U (2 x 16 doubles per slab) live in
-//    registers, q rows are loaded one group ahead.  CTAs never communicate; a CTA walks its slabs in
-//    rounds of up to 16.
+//    registers.  Its rows of q arrive through a private 6-stage shared-memory ring filled by its own
+//    cp.async copies four items ahead (no register is tied up by a load in flight, and no scoreboard is
+//    shared between the q stream and the B-fragment loads); updated rows go back to global memory
+//    straight from the C fragments.  CTAs never communicate; a CTA walks its slabs in rounds of up to 16.
 // Wasted tensor work: only the zero upper triangle of the first 64 rows of each block (0.2 % at
 // N = 32768) and the 64 x 64 T product per pass.
 #pragma once
@@ -41,11 +43,16 @@ struct B2fCfg {
     static constexpr int S = 18;                      // smem row stride per reflector (doubles): S/2 odd
     static constexpr int PANEL = NB * S;              // doubles per panel tile
     static constexpr int STAGE_DOUBLES = 2 * PANEL;   // panel 0: block P (update), panel 1: block P-1 (dot)
-    static constexpr int NS = 8, LGNS = 3, LAG = 4;
+    static constexpr int NS = 4, LGNS = 2, LAG = 2;   // V ring (shared by the CTA)
     static constexpr int NW = 8;                      // warps per CTA
     static constexpr int NGMAX = 2;                   // slabs per warp
-    static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
+    static constexpr int QS = 18;                     // q tile: [column][QS doubles], QS/2 odd
+    static constexpr int QTILE = 8 * NGMAX * QS;      // doubles per q tile (one warp, one item)
+    static constexpr int NSQ = 6, DQ = 4;             // q ring per warp: stages, items fetched ahead (DQ <= 4, see b2f_consume)
+    static constexpr int OFF_Q = NS * STAGE_DOUBLES * 8;
+    static constexpr int OFF_BAR = OFF_Q + NW * NSQ * QTILE * 8;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
 struct B2fArgs {
@@ -181,19 +188,7 @@ __device__ __forceinline__ void b2f_stage(const B2fArgs &a, double *stage, uint3
     cp_async_mbar_arrive_noinc_wy(bar_full);
 }
 
-// q rows 16 g + 4 r .. + 3 of this lane's column
-__device__ __forceinline__ void b2f_load4(const B2fArgs &a, const double *colp, bool colok, int64_t row, bool fast,
-                                          double (&y)[4])
-{
-    if (fast) {
-        const double2 u = *reinterpret_cast<const double2 *>(colp + row);
-        const double2 w = *reinterpret_cast<const double2 *>(colp + row + 2);
-        y[0] = u.x, y[1] = u.y, y[2] = w.x, y[3] = w.y;
-        return;
-    }
-#pragma unroll
-    for (int e = 0; e < 4; ++e) y[e] = (colok && row + e < a.N) ? colp[row + e] : 0.0;
-}
+// q rows 16 g + 4 r .. + 3 of this lane's column go back to global memory from the C fragments
 __device__ __forceinline__ void b2f_store4(const B2fArgs &a, double *colp, bool colok, int64_t row, bool fast,
                                            const double (&y)[4])
 {
@@ -207,14 +202,58 @@ __device__ __forceinline__ void b2f_store4(const B2fArgs &a, double *colp, bool 
         if (colok && row + e < a.N) colp[row + e] = y[e];
 }
 
+// One warp's 16-row tile of q (8 NG columns) into its private shared-memory tile [column][QS doubles]:
+// BYTES = 16 (q base and ldq*8 16-byte aligned) or 8.  Lanes run along the 128 bytes of a column; zero fill
+// beyond N and beyond nev.
+template <int NG, int BYTES>
+__device__ __forceinline__ void b2f_fetch_q(const B2fArgs &a, double *tile, int64_t col0, int64_t g, int lane)
+{
+    constexpr int QS = B2fCfg::QS;
+    constexpr int CPC = 128 / BYTES;                  // chunks per column
+    constexpr int CPI = 32 / CPC;                     // columns per instruction
+    const int ch = lane % CPC, cq = lane / CPC;
+    const int64_t row = (g << 4) + ch * (BYTES / 8);
+    const bool rows_full = (g << 4) + 16 <= a.N;
+    const bool cols_full = col0 + 8 * NG <= a.nev;
+    const double *src = a.q + (col0 + cq) * a.ldq + row;
+    const uint32_t dst = smem_u32(tile + cq * QS + ch * (BYTES / 8));
+    const int64_t ldc = a.ldq * CPI;
+    if (rows_full && cols_full) {
+#pragma unroll
+        for (int t = 0; t < 8 * NG / CPI; ++t) {
+            if (BYTES == 16)
+                cp_async16(dst + t * (CPI * QS * 8), src, 16u);
+            else
+                cp_async8(dst + t * (CPI * QS * 8), src, 8u);
+            src += ldc;
+        }
+    } else {
+        uint32_t nbytes = 0;
+        if (BYTES == 16)
+            nbytes = (row + 1 < a.N) ? 16u : (row < a.N ? 8u : 0u);
+        else
+            nbytes = (row < a.N) ? 8u : 0u;
+#pragma unroll
+        for (int t = 0; t < 8 * NG / CPI; ++t) {
+            const bool ok = (col0 + cq + t * CPI < a.nev) && nbytes;
+            if (BYTES == 16)
+                cp_async16(dst + t * (CPI * QS * 8), ok ? src : a.q, ok ? nbytes : 0u);
+            else
+                cp_async8(dst + t * (CPI * QS * 8), ok ? src : a.q, ok ? nbytes : 0u);
+            src += ldc;
+        }
+    }
+}
+
 // ---- a warp with NG slabs of 8 columns, all passes ---------------------------------------------------------
 template <int NG>
-__device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *smem, const int lane, const int member,
-                                            const int nmem, const int64_t col0, uint32_t &it, int &duty)
+__device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *smem, const int lane, const int warp,
+                                            const int member, const int nmem, const int64_t col0)
 {
     using C = B2fCfg;
-    constexpr int NB = C::NB, S = C::S, NSP = C::NS, LAG = C::LAG;
+    constexpr int NB = C::NB, S = C::S, NSP = C::NS, LAG = C::LAG, QS = C::QS, NSQ = C::NSQ, DQ = C::DQ;
     double *ring = reinterpret_cast<double *>(smem);
+    double *qring = reinterpret_cast<double *>(smem + C::OFF_Q) + (size_t)warp * NSQ * C::QTILE;
     const uint32_t bar_full = smem_u32(smem + C::OFF_BAR);
     const uint32_t bar_empty = bar_full + C::NS * 8;
     const int gq = lane >> 2, r = lane & 3;
@@ -227,67 +266,70 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
     const bool allcols = a.align16 && (col0 + 8 * NG <= a.nev);
 
-    // staging cursor: item it + NSP - LAG of the sequence (every warp of the CTA keeps its own copy)
-    B2fCursor pc = {npb, b2f_glo(npb, a.nbw)};
-    auto advance = [&]() {
-        if (pc.P < 0) return;
-        if (pc.g < ghi) {
-            ++pc.g;
+    // two cursors into the item sequence, kept identically by every warp of the CTA: pc = the V tile the
+    // warp on duty stages now (item it + NSP - LAG), qc = the q tile this warp fetches now (item it + DQ)
+    B2fCursor pc = {npb, b2f_glo(npb, a.nbw)}, qc = pc;
+    auto advance = [&](B2fCursor &c) {
+        if (c.P < 0) return;
+        if (c.g < ghi) {
+            ++c.g;
         } else {
-            --pc.P;
-            pc.g = b2f_glo(pc.P, a.nbw);
+            --c.P;
+            c.g = b2f_glo(c.P, a.nbw);
         }
     };
-    auto stage_cursor = [&](uint32_t st) {
-        b2f_stage(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pc.P, pc.g, npb, lane);
+    auto fetch_q = [&](int qst) {
+        if (qc.P >= 0) {
+            if (a.align16)
+                b2f_fetch_q<NG, 16>(a, qring + qst * C::QTILE, col0, qc.g, lane);
+            else
+                b2f_fetch_q<NG, 8>(a, qring + qst * C::QTILE, col0, qc.g, lane);
+        }
+        cp_async_commit();                              // one group per item, empty past the end
+        advance(qc);
     };
-    // prologue of this round: items 0 .. NSP-LAG-1 (the ring is drained between rounds, see the kernel)
+    uint32_t it = 0;
+    int duty = 0, qst_in = 0, qst_out = 0;              // q ring positions of item it + DQ / item it
+    // prologue: V tiles of items 0 .. NSP-LAG-1 into fresh stages, q tiles of items 0 .. DQ-1
     for (int i = 0; i < NSP - LAG; ++i) {
-        const uint32_t seq = it + i;
-        if (duty == member && pc.P >= 0) {
-            const uint32_t st = seq & (NSP - 1);
-            if (seq >= (uint32_t)NSP) mbar_wait(bar_empty + 8 * st, ((seq - NSP) >> C::LGNS) & 1);
-            stage_cursor(st);
-        }
-        advance();
+        if (duty == member && pc.P >= 0)
+            b2f_stage(a, ring + i * C::STAGE_DOUBLES, bar_full + 8 * i, pc.P, pc.g, npb, lane);
+        advance(pc);
         duty = (duty + 1 == nmem) ? 0 : duty + 1;
     }
+    for (int i = 0; i < DQ; ++i) {
+        fetch_q(qst_in);
+        qst_in = (qst_in + 1 == NSQ) ? 0 : qst_in + 1;
+    }
 
-    double W[NG][8][2], U[NG][8][2], YA[NG][4], YB[NG][4];
+    double W[NG][8][2], U[NG][8][2];
 #pragma unroll
     for (int s = 0; s < NG; ++s)
 #pragma unroll
         for (int i = 0; i < 8; ++i) W[s][i][0] = W[s][i][1] = U[s][i][0] = U[s][i][1] = 0.0;
 
-    auto load_group = [&](int64_t g, double (&T)[NG][4]) {
-        const int64_t row = (g << 4) + 4 * r;
-        const bool fast = allcols && ((g << 4) + 16 <= N);        // warp-uniform
-#pragma unroll
-        for (int s = 0; s < NG; ++s) b2f_load4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, T[s]);
-    };
-
-    // one item (pass P, group g): Y = its rows of q on entry; Yn receives the next item's rows (loaded
-    // one item ahead into the other buffer, so no register copy ever waits for the load)
-    auto do_item = [&](const int64_t P, const int64_t g, double (&Y)[NG][4], double (&Yn)[NG][4]) {
-        // --- the rows of q that item it + NSP - LAG (the staging cursor) will read go to L2 now: q streams from
-        //     DRAM one 128-byte line per column and item, and a register load issued one item ahead does
-        //     not cover that latency (20 % of the issue slots stalled on it) -- an L2 hit it does
-        if (pc.P >= 0 && allcols) {
-            const double *pp = cb + (pc.g << 4) + 4 * r;
-#pragma unroll
-            for (int s = 0; s < NG; ++s) asm volatile("prefetch.global.L2 [%0];" ::"l"(pp + s * ldq8));
-        }
-        // --- staging duty (rotates over the warps of the CTA, bt_wy.cuh)
+    int64_t P = npb, g = b2f_glo(npb, a.nbw);
+    while (P >= 0) {
+        // --- staging duty for the V ring (rotates over the warps of the CTA, bt_wy.cuh)
         {
             const uint32_t seq = it + NSP - LAG;
             if (duty == member && pc.P >= 0) {
                 const uint32_t st = seq & (NSP - 1);
                 if (seq >= (uint32_t)NSP) mbar_wait(bar_empty + 8 * st, ((seq - NSP) >> C::LGNS) & 1);
-                stage_cursor(st);
+                b2f_stage(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pc.P, pc.g, npb, lane);
             }
-            advance();
+            advance(pc);
             duty = (duty + 1 == nmem) ? 0 : duty + 1;
         }
+        // --- this warp's q tile of item it + DQ (its stage was read DQ - NSQ items ago; the __syncwarp at the
+        //     end of every item orders those reads before these copies).  Rows an earlier pass wrote were
+        //     written by lanes of this warp at least one __syncwarp ago, and a tile fetched ahead across a
+        //     pass boundary holds one of the first DQ <= 4 groups of the next pass: rows above block P, which
+        //     the pass in flight does not write.
+        fetch_q(qst_in);
+        qst_in = (qst_in + 1 == NSQ) ? 0 : qst_in + 1;
+        asm volatile("cp.async.wait_group %0;" ::"n"(DQ) : "memory");      // the tile of item `it` has landed (own copies)
+        __syncwarp();                                                     // ... and every other lane's
         const uint32_t st = it & (NSP - 1), ph = (it >> C::LGNS) & 1;
         mbar_wait(bar_full + 8 * st, ph);
         const double *pa = ring + st * C::STAGE_DOUBLES;      // V_P tile
@@ -295,9 +337,22 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
         const bool has_upd = (P < npb) && ((g << 4) >= P * NB + a.nbw);   // warp-uniform
         const bool has_dot = P >= 1;
 
+        // --- rows 4r .. 4r+3 of column gq of every slab: n-tile 0 = rows 2n (C fragment Y0 = rows 4r, 4r+2),
+        //     n-tile 1 = rows 2n+1 (Y1 = rows 4r+1, 4r+3)
+        double Y0[NG][2], Y1[NG][2];
+        {
+            const double *qt = qring + qst_out * C::QTILE + gq * QS + 4 * r;
+#pragma unroll
+            for (int s = 0; s < NG; ++s) {
+                const double2 u = *reinterpret_cast<const double2 *>(qt + 8 * s * QS);
+                const double2 w = *reinterpret_cast<const double2 *>(qt + 8 * s * QS + 2);
+                Y0[s][0] = u.x, Y1[s][0] = u.y, Y0[s][1] = w.x, Y1[s][1] = w.y;
+            }
+        }
+        qst_out = (qst_out + 1 == NSQ) ? 0 : qst_out + 1;
+
         if (has_upd) {
-            // --- q^T += U^T V_P^T: K = 64 reflectors, chunk (i, e): k-slot r = reflector 8i + 2r + e;
-            //     n-tile 0 = rows 2n (C = Y[0], Y[2]), n-tile 1 = rows 2n + 1 (C = Y[1], Y[3])
+            // --- q^T += U^T V_P^T: K = 64 reflectors, chunk (i, e): k-slot r = reflector 8i + 2r + e
             const double *bp = pa + (2 * r) * S + 2 * gq;
 #pragma unroll
             for (int i = 0; i < 8; ++i)
@@ -306,25 +361,11 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
                     const double2 b = *reinterpret_cast<const double2 *>(bp + (8 * i + e) * S);
 #pragma unroll
                     for (int s = 0; s < NG; ++s) {
-                        dmma884(Y[s][0], Y[s][2], U[s][i][e], b.x, Y[s][0], Y[s][2]);
-                        dmma884(Y[s][1], Y[s][3], U[s][i][e], b.y, Y[s][1], Y[s][3]);
+                        dmma884(Y0[s][0], Y0[s][1], U[s][i][e], b.x, Y0[s][0], Y0[s][1]);
+                        dmma884(Y1[s][0], Y1[s][1], U[s][i][e], b.y, Y1[s][0], Y1[s][1]);
                     }
                 }
         }
-        // --- the next item's rows of q go into the other buffer (if an earlier pass touched them, this same
-        //     lane wrote them).  Issued HERE, after the first use of this item's rows: issued at the top of
-        //     the item, the loads shared a scoreboard with the loads of the item before, and the first
-        //     use of Y then waited for the loads just issued (a full L2/DRAM latency per item).
-        asm volatile("" ::: "memory");
-        {
-            int64_t gn = g + 1, Pn = P;
-            if (gn > ghi) {
-                Pn = P - 1;
-                gn = b2f_glo(Pn, a.nbw);
-            }
-            if (Pn >= 0) load_group(gn, Yn);
-        }
-        asm volatile("" ::: "memory");
         if (has_dot) {
             // --- W^T += q^T V_{P-1}: K = 16 rows, chunk e: k-slot r = row 4r + e; n-tile i = reflectors 8i + n.
             //     Two n-tiles at a time: 2 NG independent accumulators in rotation
@@ -341,8 +382,10 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
 #pragma unroll
                     for (int d = 0; d < 2; ++d)
 #pragma unroll
-                        for (int s = 0; s < NG; ++s)
-                            dmma884(W[s][i + d][0], W[s][i + d][1], Y[s][e], bv[d][e], W[s][i + d][0], W[s][i + d][1]);
+                        for (int s = 0; s < NG; ++s) {
+                            const double ya = (e == 0) ? Y0[s][0] : (e == 1) ? Y1[s][0] : (e == 2) ? Y0[s][1] : Y1[s][1];
+                            dmma884(W[s][i + d][0], W[s][i + d][1], ya, bv[d][e], W[s][i + d][0], W[s][i + d][1]);
+                        }
             }
         }
         __syncwarp();
@@ -351,7 +394,10 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
             const int64_t row = (g << 4) + 4 * r;
             const bool fast = allcols && ((g << 4) + 16 <= N);    // warp-uniform
 #pragma unroll
-            for (int s = 0; s < NG; ++s) b2f_store4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, Y[s]);
+            for (int s = 0; s < NG; ++s) {
+                const double y[4] = {Y0[s][0], Y1[s][0], Y0[s][1], Y1[s][1]};
+                b2f_store4(a, cb + s * ldq8, 8 * s < ncolrem, row, fast, y);
+            }
         }
         ++it;
         if (has_dot && g == ghi) {
@@ -383,33 +429,20 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
 #pragma unroll
                 for (int i = 0; i < 8; ++i) W[s][i][0] = W[s][i][1] = 0.0;
         }
-    };
-
-    // the item sequence, two items per trip so that the q buffers alternate
-    int64_t P = npb, g = b2f_glo(npb, a.nbw);
-    auto next = [&]() {
         if (g < ghi) {
             ++g;
         } else {
             --P;
             g = b2f_glo(P, a.nbw);
         }
-    };
-    load_group(g, YA);
-    while (P >= 0) {
-        do_item(P, g, YA, YB);
-        next();
-        if (P < 0) break;
-        do_item(P, g, YB, YA);
-        next();
     }
+    asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
 // ---- the kernel ----------------------------------------------------------------------------------------------
 // grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid) and walks them in rounds of up to NW*NGMAX = 16;
 // in a round warp w takes n/8 slabs, +1 for the first n%8 warps (warps w and w+4 share a sub-partition).
-// All warps of the CTA traverse the same item sequence per round (also warps without a slab: they keep
-// the ring's duty rotation and empty-barrier counts simple), so a round is one full sequence of passes.
+// A round is one full sequence of passes; the V ring is drained and re-initialised between rounds.
 __global__ void __launch_bounds__(256, 1) bt_b2f_kernel(const B2fArgs a)
 {
     using C = B2fCfg;
@@ -438,15 +471,13 @@ __global__ void __launch_bounds__(256, 1) bt_b2f_kernel(const B2fArgs a)
             mbar_fence_init();
         }
         __syncthreads();
-        uint32_t it = 0;
-        int duty = 0;
         const int base = (int)(nround / C::NW), extra = (int)(nround % C::NW);
         const int ng = base + (warp < extra ? 1 : 0);
         const int64_t wslab0 = slab0 + done + (int64_t)warp * base + (warp < extra ? warp : extra);
         if (ng == 2)
-            b2f_consume<2>(a, smem, lane, warp, nact, wslab0 << 3, it, duty);
+            b2f_consume<2>(a, smem, lane, warp, warp, nact, wslab0 << 3);
         else if (ng == 1)
-            b2f_consume<1>(a, smem, lane, warp, nact, wslab0 << 3, it, duty);
+            b2f_consume<1>(a, smem, lane, warp, warp, nact, wslab0 << 3);
         done += nround;
         __syncthreads();                                                   // ring drained before it is re-initialised
     }
