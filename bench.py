@@ -355,7 +355,7 @@ def run_b2f_reference(args, rank: int) -> None:
 
 
 def run_b2f(args, rank, world, local_rank, dist) -> None:
-    """--step 6e: SURVEY.md 8(f) NEXT-2.  One step = one call of ``elpa2_trans_ev_band_to_full_d`` over the
+    """--step 6e: SURVEY.md 8(f) NEXT-2.  One step = one call of ``elpa2_trans_ev_band_to_full_{d,z}`` over the
     whole N x nev block (T-factor prepass + the fused DMMA kernel).  Reflectors: the seeded synthetic
     unitary set in the Eq. 6e layout (the oracle's O(N^3) full -> band reduction is out of reach at these
     sizes); q i.i.d. N(0,1); both generated on the device.  N > 1: column shards, no collective."""
@@ -364,8 +364,6 @@ def run_b2f(args, rank, world, local_rank, dist) -> None:
     from paper_2002_10991_b200 import binding, shard, synth_inputs as si
 
     cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
-    if cplx:
-        raise SystemExit("--step 6e: the complex path is not built yet")
     esz = 16 if cplx else 8
     Nv = max(N - nbw - 1, 0)
     flops = b2f_flops(cplx, N, nbw, nev)
@@ -461,7 +459,7 @@ def run_b2f(args, rank, world, local_rank, dist) -> None:
                                         "MEASURED_PEAKS.json has no FP64 figure",
                          "peak_dfma_probe": dfma_tf, "peak_dmma_probe": dmma_tf, "peak_nominal": NOMINAL_FP64_TFLOPS,
                          "frac_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                         "kernel": "bt_b2f_kernel (the interval also holds its T-factor prepass kernel)",
+                         "kernel": ("bt_b2fz_kernel" if cplx else "bt_b2f_kernel") + " (the interval also holds its T-factor prepass kernel)",
                          "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
                          "traffic": traffic, "traffic_profile": traffic_profile},
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
@@ -486,7 +484,7 @@ def main() -> None:
                     help="time SURVEY 8(f) NEXT-1 instead: the GPU bulge chase (real configs) that produces the reflectors")
     ap.add_argument("--step", default="6d", choices=["6d", "6e"],
                     help="6d (default): tridiagonal -> band back-transformation, the north star; 6e: SURVEY 8(f) NEXT-2, "
-                         "band -> full back-transformation on the same config's N, nbw, nev (real configs)")
+                         "band -> full back-transformation on the same config's N, nbw, nev")
     ap.add_argument("--nev-frac", type=float, default=None,
                     help="partial spectrum (PAPER.md:218): replace nev by round(frac * N)")
     ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",

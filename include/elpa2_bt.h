@@ -36,8 +36,9 @@
  *
  * Return value: 0 on success; -i if the i-th argument (1-based: N=1, nbw=2, nev=3, hh_v=4,
  * hh_tau=5, q=6, ldq=7, stream=8) is invalid; > 0 is the cudaError_t of a failed launch.
- * Invalid: N < 0; nbw not in {32, 64, 128} ("32, 64, and 128 being the recommended
- * choices"); nev < 0; a NULL pointer when there is work to do; ldq < max(N,1); a q or hh_v pointer
+ * Invalid: N < 0; nbw not a multiple of 32 in [32, 256] (real) / [32, 160] (complex: the planar window
+ * of 8 columns must fit in 255 registers) -- PAPER.md:186: "multiples of 32 ... 32, 64, and 128 being
+ * the recommended choices"; variant 2 and the bulge chase take 32, 64, 128 only; nev < 0; a NULL pointer when there is work to do; ldq < max(N,1); a q or hh_v pointer
  * that is not aligned to its element size, hh_v not 16-byte aligned (bulk-copy requirement).
  * N <= 1 or nev == 0 is success with no work.  Nothing is printed, no errno, no exceptions.
  */
@@ -116,10 +117,17 @@ int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau,
 int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv,
                                   const double *tau, double *q, int64_t ldq, void *stream);
 
+/* Complex FP64 (interleaved (re, im) doubles; ldv, ldq count complex elements): H_j = I - tau_j v_j v_j^H
+ * with tau as stored and v^H conjugated in the dot product (R2).  Same layout, same argument positions
+ * and error codes; hv, tau and q must be 16-byte aligned, ldv >= N (no parity requirement).  The -T
+ * factors take 64 KB per block of 64 reflectors from the scratch pool. */
+int elpa2_trans_ev_band_to_full_z(int64_t N, int nbw, int64_t nev, const void *hv, int64_t ldv,
+                                  const void *tau, void *q, int64_t ldq, void *stream);
+
 /* Same operation with HOST buffers (pageable or pinned), synchronous: H2D of hv, tau and q, the two
  * kernels, D2H of q (what bench.py --step 6e reports as e2e).  Device scratch cached as for
  * elpa2_trans_ev_tridi_to_band_host.  Argument positions: is_complex=1, N=2, nbw=3, nev=4, hv=5, ldv=6,
- * tau=7, q=8, ldq=9.  is_complex must be 0 (the complex path has the device entry point only). */
+ * tau=7, q=8, ldq=9. */
 int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hv,
                                      int64_t ldv, const void *tau, void *q, int64_t ldq);
 
@@ -146,6 +154,11 @@ int elpa2_hh_blocks(int64_t N, int nbw, int64_t s);
  * previous variant or -1 if `variant` is unknown. */
 int elpa2_bt_last_launch_count(void);
 int elpa2_bt_set_variant(int variant);
+/* Testing aid (per thread): force the number P of warps that share a slab of 8 columns on interleaved
+ * chains in the default variant (DESIGN.md 5.1 "chain-parallel mode"; R5 makes every P give the same
+ * result): 0 = as planned, 1, 2 or 4 (complex: 4 runs as 2).  tests/test_gpu_ordering.py compares the
+ * results bit for bit across P.  Returns the previous value or -1. */
+int elpa2_bt_set_chain_parallel(int P);
 
 /* Launch plan of the default variant's main kernel for a problem on a device with n_sm SMs (host, pure
  * integer arithmetic, no device needed; DESIGN.md 5.1 "Decomposition"): out = { CTAs, warps per CTA,

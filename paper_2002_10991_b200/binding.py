@@ -22,8 +22,8 @@ EXPORTS = (
     "elpa2_trans_ev_tridi_to_band_host", "elpa2_hh_count", "elpa2_hh_offset", "elpa2_hh_blocks",
     "elpa2_bt_last_launch_count", "elpa2_bt_set_variant", "elpa2_bt_version", "elpa2_bt_probe_fp64",
     "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
-    "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d",
-    "elpa2_trans_ev_band_to_full_host",
+    "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z",
+    "elpa2_trans_ev_band_to_full_host", "elpa2_bt_set_chain_parallel",
 )
 
 
@@ -56,8 +56,9 @@ def lib() -> ctypes.CDLL:
         for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
             getattr(L, nm).argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
             getattr(L, nm).restype = i32
-        L.elpa2_trans_ev_band_to_full_d.argtypes = [i64, i32, i64, vp, i64, vp, vp, i64, vp]
-        L.elpa2_trans_ev_band_to_full_d.restype = i32
+        for nm in ("elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z"):
+            getattr(L, nm).argtypes = [i64, i32, i64, vp, i64, vp, vp, i64, vp]
+            getattr(L, nm).restype = i32
         L.elpa2_trans_ev_band_to_full_host.argtypes = [i32, i64, i32, i64, vp, i64, vp, vp, i64]
         L.elpa2_trans_ev_band_to_full_host.restype = i32
         L.elpa2_bt_release_scratch.argtypes = []
@@ -76,6 +77,8 @@ def lib() -> ctypes.CDLL:
         L.elpa2_bt_last_launch_count.restype = i32
         L.elpa2_bt_set_variant.argtypes = [i32]
         L.elpa2_bt_set_variant.restype = i32
+        L.elpa2_bt_set_chain_parallel.argtypes = [i32]
+        L.elpa2_bt_set_chain_parallel.restype = i32
         L.elpa2_bt_version.argtypes = []
         L.elpa2_bt_version.restype = ctypes.c_char_p
         L.elpa2_bt_probe_fp64.argtypes = [i32, i32, i32, ctypes.POINTER(ctypes.c_double)]
@@ -138,6 +141,11 @@ def version() -> str:
 
 def set_variant(variant: int) -> int:
     return lib().elpa2_bt_set_variant(variant)
+
+
+def set_chain_parallel(P: int) -> int:
+    """Testing aid: force P warps per slab (0 = planned); see include/elpa2_bt.h."""
+    return lib().elpa2_bt_set_chain_parallel(P)
 
 
 def last_launch_count() -> int:
@@ -205,8 +213,9 @@ def trans_ev_band_to_full(N: int, nbw: int, hv, tau, q, stream=None) -> None:
 
     if not (q.is_cuda and hv.is_cuda and tau.is_cuda):
         raise ValueError("device tensors required")
-    if q.dtype != torch.float64 or hv.dtype != q.dtype or tau.dtype != q.dtype:
-        raise ValueError("float64 throughout")
+    if q.dtype not in (torch.float64, torch.complex128) or hv.dtype != q.dtype or tau.dtype != q.dtype:
+        raise ValueError("float64 or complex128 throughout")
+    cplx = q.dtype == torch.complex128
     Nv = max(N - nbw - 1, 0)
     if q.dim() != 2 or q.shape[0] != N or (N > 1 and q.stride(0) != 1):
         raise ValueError("q must be (N, nev) column-major")
@@ -217,8 +226,8 @@ def trans_ev_band_to_full(N: int, nbw: int, hv, tau, q, stream=None) -> None:
     ldv = hv.stride(1) if Nv > 1 else max(N + (N & 1), 2)
     if not (hv.device == q.device and tau.device == q.device and torch.cuda.current_device() == q.device.index):
         raise ValueError("hv, tau and q must live on the current CUDA device")
-    rc = lib().elpa2_trans_ev_band_to_full_d(N, nbw, nev, hv.data_ptr(), ldv, tau.data_ptr(), q.data_ptr(), ldq,
-                                             _stream_ptr(stream))
+    fn = lib().elpa2_trans_ev_band_to_full_z if cplx else lib().elpa2_trans_ev_band_to_full_d
+    rc = fn(N, nbw, nev, hv.data_ptr(), ldv, tau.data_ptr(), q.data_ptr(), ldq, _stream_ptr(stream))
     if rc != 0:
         raise Elpa2BtError(rc)
 
@@ -228,14 +237,14 @@ def trans_ev_band_to_full_host(N: int, nbw: int, hv, tau, q) -> None:
     reflectors (ldv = hv.shape[0] even), ``tau`` (Nv,), ``q`` Fortran-ordered (N, nev), updated in place."""
     import numpy as np
 
-    if np.iscomplexobj(q) or q.dtype != np.float64 or hv.dtype != np.float64 or tau.dtype != np.float64:
-        raise ValueError("float64 throughout")
+    if q.dtype not in (np.float64, np.complex128) or hv.dtype != q.dtype or tau.dtype != q.dtype:
+        raise ValueError("float64 or complex128 throughout")
     Nv = max(N - nbw - 1, 0)
     if q.ndim != 2 or q.shape[0] != N or not q.flags.f_contiguous:
         raise ValueError("q must be Fortran-contiguous (N, nev)")
     if Nv > 0 and (hv.ndim != 2 or hv.shape[1] != Nv or hv.shape[0] < N or not hv.flags.f_contiguous):
         raise ValueError("hv must be Fortran-contiguous (ldv >= N, Nv)")
-    rc = lib().elpa2_trans_ev_band_to_full_host(0, N, nbw, q.shape[1], hv.ctypes.data, hv.shape[0], tau.ctypes.data,
+    rc = lib().elpa2_trans_ev_band_to_full_host(int(np.iscomplexobj(q)), N, nbw, q.shape[1], hv.ctypes.data, hv.shape[0], tau.ctypes.data,
                                                 q.ctypes.data, max(N, 1))
     if rc != 0:
         raise Elpa2BtError(rc)

@@ -36,7 +36,7 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
     if (r1 > N - 1) r1 = N - 1;
     const int L = (int)(r1 - r0 + 1);
     const int64_t c = (k == 0) ? s : r0 - NBW;
-    const int64_t g = hh_off(N, LG, s) + k;
+    const int64_t g = hh_off(N, NBW, s) + k;
 #define BC_B(i, j) ab[((i) - (j)) + (j) * ldab]
     double *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {                       // nothing to eliminate: identity slot (R3)
@@ -217,7 +217,7 @@ __device__ __forceinline__ bool bc_step_smem(const int64_t N, const int64_t s, c
     if (r1 > N - 1) r1 = N - 1;
     const int L = (int)(r1 - r0 + 1);
     const int64_t c = (k == 0) ? s : r0 - NBW;
-    const int64_t g = hh_off(N, LG, s) + k;
+    const int64_t g = hh_off(N, NBW, s) + k;
     double *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {
         for (int i = tid; i < NBW; i += nt) vout[i] = (i == 0) ? 1.0 : 0.0;
@@ -498,7 +498,7 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
     if (r1 > N - 1) r1 = N - 1;
     const int L = (int)(r1 - r0 + 1);
     const int64_t c = (k == 0) ? s : r0 - NBW;
-    const int64_t g = hh_off(N, LG, s) + k;
+    const int64_t g = hh_off(N, NBW, s) + k;
 #define BC_Z(i, j) ab[((i) - (j)) + (j) * ldab]
     zc *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {
@@ -679,7 +679,7 @@ __device__ __forceinline__ bool bc_step_smem_z(const int64_t N, const int64_t s,
     if (r1 > N - 1) r1 = N - 1;
     const int L = (int)(r1 - r0 + 1);
     const int64_t c = (k == 0) ? s : r0 - NBW;
-    const int64_t g = hh_off(N, LG, s) + k;
+    const int64_t g = hh_off(N, NBW, s) + k;
     zc *vout = hh_v + g * NBW;
     if (k > 0 && L == 1) {
         for (int i = tid; i < NBW; i += nt) vout[i] = {(i == 0) ? 1.0 : 0.0, 0.0};

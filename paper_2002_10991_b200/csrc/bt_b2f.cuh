@@ -55,13 +55,16 @@ struct B2fCfg {
     static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
+// N, ldq and ldv count DOUBLES per column (= elements x ew): the complex kernel (bt_b2fz.cuh) sees its
+// interleaved N x Nv matrix as a real 2N x Nv one, so staging, the q ring and the tile stores are shared.
 struct B2fArgs {
     int64_t N, nev, ldq, ldv, Nv;
-    int nbw;
+    int nbw;               // in elements
+    int ew;                // doubles per element: 1 real, 2 complex
     const double *hv;      // N x Nv column-major, ldv
-    const double *tneg;    // npb x 64 x 64, row-major: tneg[p][i][k] = -T_p[i][k]
+    const double *tneg;    // npb x 64 x 64 elements, row-major: tneg[p][i][k] = -T_p[i][k]
     double *q;
-    int align16;           // q base and ldq*8 are 16-byte aligned
+    int align16;           // q base and ldq*8 are 16-byte aligned (always 1 for complex)
 };
 
 __host__ __device__ __forceinline__ int64_t b2f_nblocks(int64_t Nv) { return (Nv + B2fCfg::NB - 1) / B2fCfg::NB; }
@@ -143,10 +146,10 @@ __global__ void __launch_bounds__(256) b2f_tfactor_kernel(int64_t N, int64_t Nv,
 struct B2fCursor {
     int64_t P, g;
 };
-__device__ __forceinline__ int64_t b2f_glo(int64_t P, int nbw)
+__device__ __forceinline__ int64_t b2f_glo(int64_t P, int nbw, int ew = 1)
 {
     const int64_t pb = P >= 1 ? P - 1 : 0;
-    return (pb * B2fCfg::NB + nbw) >> 4;
+    return ((pb * B2fCfg::NB + nbw) * ew) >> 4;
 }
 
 // stage one item (whole warp): panel 0 = V_P rows of group g (if the group is inside block P),
@@ -165,7 +168,7 @@ __device__ __forceinline__ void b2f_stage(const B2fArgs &a, double *stage, uint3
 #pragma unroll
     for (int panel = 0; panel < 2; ++panel) {
         const int64_t blk = P - panel;
-        const bool on = (panel == 0) ? (P < npb && row0 >= P * NB + a.nbw) : (P >= 1);
+        const bool on = (panel == 0) ? (P < npb && row0 >= (P * NB + a.nbw) * a.ew) : (P >= 1);
         if (!on) continue;                            // warp-uniform
         const double *src = a.hv + row + (blk * NB + lr) * a.ldv;
         const uint32_t dst = smem_u32(stage + panel * B2fCfg::PANEL + lr * S + 2 * ch);
@@ -513,6 +516,7 @@ inline cudaError_t launch_b2f(int64_t N, int nbw, int64_t nev, const double *hv,
     a.ldv = ldv;
     a.Nv = Nv;
     a.nbw = nbw;
+    a.ew = 1;
     a.hv = hv;
     a.tneg = tneg;
     a.q = q;

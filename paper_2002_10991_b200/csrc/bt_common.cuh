@@ -7,15 +7,16 @@
 namespace elpa2bt {
 
 // ---- reflector slot layout (include/elpa2_bt.h; R3) --------------------------------
-// F(x) = sum_{y=1..x} ceil(y / nbw);  off(s) = F(N-1) - F(N-1-s);  nbw = 1 << lg.
-__host__ __device__ __forceinline__ int64_t hh_F(int64_t x, int lg)
+// F(x) = sum_{y=1..x} ceil(y / nbw) = nbw t (t+1) / 2 + r (t+1) with x = t nbw + r;  off(s) = F(N-1) - F(N-1-s).
+// Any nbw >= 1 (the kernels pass a compile-time constant, so the division is a multiply-shift).
+__host__ __device__ __forceinline__ int64_t hh_F(int64_t x, int nbw)
 {
-    const int64_t t = x >> lg, r = x - (t << lg);
-    return ((t * (t + 1)) >> 1 << lg) + r * (t + 1);
+    const int64_t t = x / nbw, r = x - t * nbw;
+    return ((t * (t + 1)) >> 1) * nbw + r * (t + 1);
 }
-__host__ __device__ __forceinline__ int64_t hh_off(int64_t N, int lg, int64_t s)
+__host__ __device__ __forceinline__ int64_t hh_off(int64_t N, int nbw, int64_t s)
 {
-    return hh_F(N - 1, lg) - hh_F(N - 1 - s, lg);
+    return hh_F(N - 1, nbw) - hh_F(N - 1 - s, nbw);
 }
 
 // Opt-in to more than 48 KB of dynamic shared memory.  The attribute belongs to the (function, device)

@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(MAXT, 1) bt_shift_kernel(const WinArgs a)
     __syncthreads();
 
     const int64_t N = a.N;
-    const int64_t K0 = (N - 2 + NBW) >> C::LG;     // K(0) = ceil((N-1)/nbw): number of chains
+    const int64_t K0 = (N - 2 + NBW) / NBW;     // K(0) = ceil((N-1)/nbw): number of chains
     const int64_t B0 = (N - 1) >> 4;
 
     if (warp == nw) {
@@ -290,20 +290,20 @@ __global__ void __launch_bounds__(MAXT, 1) bt_shift_kernel(const WinArgs a)
         constexpr int CPLN = (NCOPY + 31) / 32;               // copies per lane
         constexpr uint32_t PBYTES = RL * C::ESZ;              // bytes per piece
         const int u = lane & 15;
-        const int64_t FN1 = hh_F(N - 1, C::LG);
+        const int64_t FN1 = hh_F(N - 1, NBW);
         uint32_t it = 0;
         for (int64_t k = 0; k < K0; ++k) {
-            const int64_t Bend = (1 + (k << C::LG)) >> 4;
+            const int64_t Bend = (1 + (k * NBW)) >> 4;
             for (int64_t B = B0; B >= Bend; --B, ++it) {
                 const uint32_t st = it % NS, ph = (it / NS) & 1;
                 mbar_wait_backoff(bar_empty + 8 * st, ph ^ 1);
                 const int64_t r0 = (B << 4) + u;
-                const int64_t s = r0 - 1 - (k << C::LG);
+                const int64_t s = r0 - 1 - (k * NBW);
                 const bool valid = (r0 <= N - 1) && (s >= 0);
                 double tr = 0.0, ti = 0.0;
                 int64_t g = 0;
                 if (valid) {
-                    g = FN1 - hh_F(N - 1 - s, C::LG) + k;
+                    g = FN1 - hh_F(N - 1 - s, NBW) + k;
                     tr = __ldg(a.hh_tau + g * EW);
                     if (CPLX) ti = __ldg(a.hh_tau + g * EW + 1);
                 }
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(MAXT, 1) bt_shift_kernel(const WinArgs a)
 #pragma unroll
             for (int i = 0; i < EW; ++i) c[j][i] = 0.0;
         }
-        const int64_t Bend = (1 + (k << C::LG)) >> 4;
+        const int64_t Bend = (1 + (k * NBW)) >> 4;
         sh_tile_fill<C, CPLX>(a, tiles + (B0 & 1) * (C::TILE_BYTES / 8), col0, B0, lane);
         cp_async_commit();
         for (int64_t B = B0; B >= Bend; --B, ++it) {

@@ -9,22 +9,21 @@
 namespace elpa2bt {
 
 template <bool CPLX>
-__global__ void __launch_bounds__(128) bt_simple_kernel(int64_t N, int lg, int64_t nev, const double *hh_v,
+__global__ void __launch_bounds__(128) bt_simple_kernel(int64_t N, int nbw, int64_t nev, const double *hh_v,
                                                          const double *hh_tau, double *q, int64_t ldq)
 {
     constexpr int EW = CPLX ? 2 : 1;
-    __shared__ double vs[128 * EW];
+    __shared__ double vs[256 * EW];                  // nbw <= 256
     __shared__ double taus[2];
-    const int nbw = 1 << lg;
     const int64_t col = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     double *x = q + (col < nev ? col : 0) * ldq * EW;
-    const int64_t FN1 = hh_F(N - 1, lg);
+    const int64_t FN1 = hh_F(N - 1, nbw);
     for (int64_t s = N - 2; s >= 0; --s) {
-        const int64_t off = FN1 - hh_F(N - 1 - s, lg);
-        const int64_t K = (N - 1 - s + nbw - 1) >> lg;
+        const int64_t off = FN1 - hh_F(N - 1 - s, nbw);
+        const int64_t K = (N - 1 - s + nbw - 1) / nbw;
         for (int64_t k = 0; k < K; ++k) {
             const int64_t g = off + k;
-            const int64_t r0 = s + 1 + (k << lg);
+            const int64_t r0 = s + 1 + k * nbw;
             int64_t L = N - r0;
             L = L > nbw ? nbw : L;
             __syncthreads();

@@ -38,23 +38,25 @@ namespace elpa2bt {
 
 template <int NBW_, int NW_ = 8>
 struct WyCfg {
-    static constexpr int NBW = NBW_;
-    static constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    static constexpr int NBW = NBW_;                  // any multiple of 16 (R13: the library instantiates multiples of 32)
+    static constexpr int NB8 = NBW / 8;               // 8-row blocks per chase block
     static constexpr int NT = NBW / 8 + 1;            // 8-row tiles in the window
     static constexpr int W = 8 * NT;                  // window rows (= nbw + 8; W % 16 == 8)
     static constexpr int NW = NW_;                    // warps per CTA: 8 (255 registers) or, for few columns, 16 (128)
-    static constexpr int NGMAX = (NW_ > 8) ? 1 : (NBW <= 64) ? 4 : 2;   // most 8-column slabs per warp
-    static constexpr int NS = (NW_ > 8) ? 16 : 8;     // ring stages
-    static constexpr int LGNS = (NW_ > 8) ? 4 : 3;
+    static constexpr int NGMAX = (NW_ > 8) ? 1 : (NBW <= 64) ? 4 : (NBW <= 128) ? 2 : 1;   // most 8-column slabs per warp
+    // ring stages: 8 (16 in the 16-warp build) while 8 stages of 16 W doubles fit, else 4
+    static constexpr int NS = (NW_ > 8) ? 16 : (8 * 16 * W * 8 <= 216 * 1024) ? 8 : 4;
+    static constexpr int LGNS = (NS == 16) ? 4 : (NS == 8) ? 3 : 2;
     static constexpr int LAG = 4;                     // staging waits for the block LAG iterations back
     static constexpr int VA_OFF = 0;                  // VA[i][w] = V, row stride W
     static constexpr int YB_OFF = 8 * W;              // YB[w][j] = (V (-T))[w][j], row stride 8
     static constexpr int STAGE_DOUBLES = 16 * W;
     static constexpr int YBLK = 8 * W;                // doubles of scratch per block (its YB image)
-    static constexpr int PW = (NBW <= 64) ? 8 : 4;    // warps (= blocks) per CTA of the prepass kernel
+    static constexpr int PW = (NBW <= 64) ? 8 : (NBW <= 128) ? 4 : 2;    // warps (= blocks) per CTA of the prepass kernel
     static constexpr int OFF_BAR = NS * STAGE_DOUBLES * 8;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
     static_assert(W % 16 == 8, "VA row stride must be 8 mod 16 doubles (bank-conflict-free LDS.128)");
+    static_assert(SMEM_BYTES <= 227 * 1024, "shared memory");
 };
 
 struct WyArgs {
@@ -72,22 +74,22 @@ struct WyArgs {
 // chain k = 0 .. K0-1 (K0 = ceil((N-1)/nbw)); within a chain, blocks b = bhi down to k*nbw/8, where
 // bhi = (N-1)/8.  id(k, b) = base(k) + (bhi - b) is the consumption order.
 __host__ __device__ __forceinline__ int64_t wy_bhi(int64_t N) { return (N - 1) >> 3; }
-__host__ __device__ __forceinline__ int64_t wy_base(int64_t N, int lg, int64_t k)
+__host__ __device__ __forceinline__ int64_t wy_base(int64_t N, int nbw, int64_t k)
 {
-    return k * (wy_bhi(N) + 1) - ((int64_t)1 << (lg - 3)) * ((k * (k - 1)) >> 1);
+    return k * (wy_bhi(N) + 1) - (int64_t)(nbw >> 3) * ((k * (k - 1)) >> 1);
 }
-__host__ __device__ __forceinline__ int64_t wy_nchains(int64_t N, int lg) { return (N - 2 + ((int64_t)1 << lg)) >> lg; }
-__host__ __device__ __forceinline__ int64_t wy_nblocks(int64_t N, int lg) { return wy_base(N, lg, wy_nchains(N, lg)); }
+__host__ __device__ __forceinline__ int64_t wy_nchains(int64_t N, int nbw) { return (N - 2 + nbw) / nbw; }
+__host__ __device__ __forceinline__ int64_t wy_nblocks(int64_t N, int nbw) { return wy_base(N, nbw, wy_nchains(N, nbw)); }
 
 // slot of reflector i of block (k, b) (first row r0 = 8b + 7 - i; sweep s = r0 - 1 - k nbw; R3),
 // -1 if the block position is outside the chain
-template <int LG>
+template <int NBW>
 __device__ __forceinline__ int64_t wy_slot(int64_t N, int64_t FN1, int64_t k, int64_t b, int i)
 {
     const int64_t r0 = (b << 3) + 7 - i;
-    const int64_t s = r0 - 1 - (k << LG);
+    const int64_t s = r0 - 1 - k * NBW;
     if (r0 > N - 1 || s < 0) return -1;
-    return FN1 - hh_F(N - 1 - s, LG) + k;
+    return FN1 - hh_F(N - 1 - s, NBW) + k;
 }
 
 __device__ __forceinline__ void dmma884(double &d0, double &d1, const double a, const double b, const double c0,
@@ -122,12 +124,12 @@ __global__ void __launch_bounds__(WyCfg<NBW>::PW * 32) wy_prepass_kernel(int64_t
     const int gq = lane >> 2, r = lane & 3;
     const int64_t k = blockIdx.y;
     const int64_t bhi = wy_bhi(N);
-    const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
+    const int64_t nblk = bhi - (k * C::NB8) + 1;
     const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
     if (j >= nblk) return;
     const int64_t b = bhi - j;
-    const int64_t FN1 = hh_F(N - 1, C::LG);
-    const int64_t slot = wy_slot<C::LG>(N, FN1, k, b, gq);
+    const int64_t FN1 = hh_F(N - 1, C::NBW);
+    const int64_t slot = wy_slot<C::NBW>(N, FN1, k, b, gq);
     const double tau = slot >= 0 ? hh_tau[slot] : 0.0;
     double s0 = 0.0, s1 = 0.0, u0 = 0.0, u1 = 0.0;
 #pragma unroll
@@ -162,7 +164,7 @@ __global__ void __launch_bounds__(WyCfg<NBW>::PW * 32) wy_prepass_kernel(int64_t
     __syncwarp();
     // Y[w][j] = sum_i V[w][i] (-T)[i][j]: M = rows of a tile, N = j, K = i (two k-chunks)
     const double tb0 = Sm[warp][r * 8 + gq], tb1 = Sm[warp][(r + 4) * 8 + gq];
-    double *out = yb + (wy_base(N, C::LG, k) + j) * C::YBLK;
+    double *out = yb + (wy_base(N, C::NBW, k) + j) * C::YBLK;
 #pragma unroll
     for (int tt = 0; tt < C::NT; ++tt) {
         double y0 = 0.0, y1 = 0.0;
@@ -180,7 +182,7 @@ __device__ __forceinline__ void wy_stage(const WyArgs &a, double *stage, uint32_
 {
     constexpr int NBW = C::NBW, W = C::W;
     const int i8 = lane & 7;
-    const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
+    const int64_t slot = wy_slot<C::NBW>(a.N, FN1, k, b, i8);
     // YB: the prepass wrote the shared-memory image; one bulk copy (TMA engine)
     if (lane == 0) {
         mbar_arrive_expect_tx(bar_full, C::YBLK * 8u);
@@ -262,9 +264,9 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const uint32_t bar_empty = bar_full + C::NS * 8;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
-    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t bhi = wy_bhi(N);
-    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq;
@@ -277,7 +279,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     // staging cursor: block it + NSP - LAG of this ring's sequence
     int64_t pk = grp, pb = bhi;
     auto advance = [&]() {
-        if (pb > (pk << (C::LG - 3))) {
+        if (pb > (pk * C::NB8)) {
             --pb;
         } else {
             pk += P;
@@ -285,7 +287,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
         }
     };
     auto stage_cursor = [&](uint32_t st) {
-        wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::LG, pk) + (bhi - pb), FN1,
+        wy_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::NBW, pk) + (bhi - pb), FN1,
                     lane);
     };
     // prologue: blocks 0 .. NSP-LAG-1 go into fresh stages
@@ -305,7 +307,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     uint32_t it = 0;                   // blocks consumed from this ring
     int duty = 0;
     for (int64_t k = grp; k < K0; k += P) {
-        const int64_t blo = k << (C::LG - 3);
+        const int64_t blo = k * C::NB8;
         // chain-parallel hand-over: chain k-1 of this slab is walked by another warp of the CTA
         const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
@@ -535,14 +537,17 @@ struct WyPlan {
 };
 inline WyPlan wy_plan(bool cplx, int nbw, int64_t N, int64_t nev, int nsm, int force_P, int force_nw)
 {
-    const int lg = nbw == 32 ? 5 : nbw == 64 ? 6 : 7;
-    const int64_t K0 = wy_nchains(N, lg);
+    const int64_t K0 = wy_nchains(N, nbw);
     WyPlan pl;
     pl.nslab = (nev + 7) >> 3;
-    const int ngmax8 = cplx ? (nbw <= 64 ? 2 : 1) : (nbw <= 64 ? 4 : 2);
+    const int ngmax8 = cplx ? (nbw <= 64 ? 2 : 1) : (nbw <= 64 ? 4 : nbw <= 128 ? 2 : 1);
     const bool many_warps = !cplx && nbw <= 64 && force_P == 0 && force_nw != 8 && pl.nslab <= (int64_t)nsm * 4 && K0 >= 16;
     pl.nwarps = many_warps ? 16 : 8;
-    pl.P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(pl.nslab, K0, nsm, 8, cplx ? 2 : 4));
+    // a chain-parallel group needs at least two ring stages of its own: P <= NS / 2
+    const int ns = cplx ? (nbw <= 64 ? 8 : 4) : ((8 * 16 * (nbw + 8) * 8 <= 216 * 1024) ? 8 : 4);
+    const int maxP = cplx ? 2 : (ns >= 8 ? 4 : 2);
+    if (force_P > maxP) force_P = maxP;
+    pl.P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(pl.nslab, K0, nsm, 8, maxP));
     // (the complex kernel and the 16-warp build walk one slab per warp in chain-parallel mode)
     pl.per_cta = (int64_t)(pl.nwarps / pl.P) * ((many_warps || (cplx && pl.P > 1)) ? 1 : ngmax8);
     const int64_t waves = (pl.nslab + nsm * pl.per_cta - 1) / (nsm * pl.per_cta);
@@ -555,12 +560,12 @@ inline WyPlan wy_plan(bool cplx, int nbw, int64_t N, int64_t nev, int nsm, int f
 template <int NBW>
 size_t wy_tn_bytes(int64_t N)
 {
-    return (size_t)wy_nblocks(N, WyCfg<NBW>::LG) * WyCfg<NBW>::YBLK * sizeof(double);
+    return (size_t)wy_nblocks(N, NBW) * WyCfg<NBW>::YBLK * sizeof(double);
 }
 template <int NBW>
 size_t wy_scratch_bytes(int64_t N, int64_t nev)
 {
-    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, WyCfg<NBW>::LG) * sizeof(uint32_t);
+    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, NBW) * sizeof(uint32_t);
     return wy_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
@@ -584,7 +589,7 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
                       int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0, int force_nw = 0)
 {
     using C = WyCfg<NBW>;
-    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t nslab = (nev + 7) >> 3;
     double *tn = (double *)scratch;
     uint32_t *prog = (uint32_t *)((char *)scratch + wy_tn_bytes<NBW>(N));

@@ -18,7 +18,7 @@ namespace elpa2bt {
 template <int NBW_>
 struct WyzCfg {
     static constexpr int NBW = NBW_;
-    static constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    static constexpr int NB8 = NBW / 8;               // 8-row blocks per chase block
     static constexpr int NT = NBW / 8 + 1;            // 8-row tiles in the window
     static constexpr int W = 8 * NT;                  // window rows
     static constexpr int NW = 8;                      // warps per CTA
@@ -55,12 +55,12 @@ __global__ void __launch_bounds__(WyzCfg<NBW>::PW * 32) wyz_prepass_kernel(int64
     const int gq = lane >> 2, r = lane & 3;
     const int64_t k = blockIdx.y;
     const int64_t bhi = wy_bhi(N);
-    const int64_t nblk = bhi - (k << (C::LG - 3)) + 1;
+    const int64_t nblk = bhi - (k * C::NB8) + 1;
     const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
     if (j >= nblk) return;
     const int64_t b = bhi - j;
-    const int64_t FN1 = hh_F(N - 1, C::LG);
-    const int64_t slot = wy_slot<C::LG>(N, FN1, k, b, gq);
+    const int64_t FN1 = hh_F(N - 1, C::NBW);
+    const int64_t slot = wy_slot<C::NBW>(N, FN1, k, b, gq);
     double taur = 0.0, taui = 0.0;
     if (slot >= 0) {
         taur = hh_tau[2 * slot];
@@ -125,7 +125,7 @@ __global__ void __launch_bounds__(WyzCfg<NBW>::PW * 32) wyz_prepass_kernel(int64
         tbr[c] = Sm[warp][((r + 4 * c) * 8 + gq) * 2];
         tbi[c] = Sm[warp][((r + 4 * c) * 8 + gq) * 2 + 1];
     }
-    double *out = yb + (wy_base(N, C::LG, k) + j) * C::YBLK;
+    double *out = yb + (wy_base(N, C::NBW, k) + j) * C::YBLK;
 #pragma unroll
     for (int tt = 0; tt < C::NT; ++tt) {
         double yr0 = 0.0, yr1 = 0.0, yi0 = 0.0, yi1 = 0.0;
@@ -156,7 +156,7 @@ __device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32
 {
     constexpr int NBW = C::NBW;
     const int i8 = lane & 7;
-    const int64_t slot = wy_slot<C::LG>(a.N, FN1, k, b, i8);
+    const int64_t slot = wy_slot<C::NBW>(a.N, FN1, k, b, i8);
     const unsigned valid = __ballot_sync(0xffffffffu, slot >= 0) & 0xffu;
     if (lane == 0) {
         mbar_arrive_expect_tx(bar_full, (uint32_t)__popc(valid) * NBW * 16u + C::YBLK * 8u);
@@ -208,9 +208,9 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     const uint32_t bar_empty = bar_full + C::NS * 8;
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
-    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t bhi = wy_bhi(N);
-    const int64_t FN1 = hh_F(N - 1, C::LG);
+    const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1 (ldq counts complex elements)
     double *const cb = a.q + (col0 + gq < a.nev ? col0 + gq : 0) * a.ldq * 2;
@@ -220,7 +220,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
 
     int64_t pk = grp, pb = bhi;                         // staging cursor: block it + NSP - LAG of this ring
     auto advance = [&]() {
-        if (pb > (pk << (C::LG - 3))) {
+        if (pb > (pk * C::NB8)) {
             --pb;
         } else {
             pk += P;
@@ -228,7 +228,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
         }
     };
     auto stage_cursor = [&](uint32_t st) {
-        wyz_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::LG, pk) + (bhi - pb), FN1,
+        wyz_stage<C>(a, ring + st * C::STAGE_DOUBLES, bar_full + 8 * st, pk, pb, wy_base(N, C::NBW, pk) + (bhi - pb), FN1,
                      lane);
     };
     for (int i = 0; i < NSP - LAG; ++i) {
@@ -242,7 +242,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     uint32_t it = 0;
     int duty = 0;
     for (int64_t k = grp; k < K0; k += P) {
-        const int64_t blo = k << (C::LG - 3);
+        const int64_t blo = k * C::NB8;
         const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
         uint32_t known = 0;
@@ -437,12 +437,12 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
 template <int NBW>
 size_t wyz_tn_bytes(int64_t N)
 {
-    return (size_t)wy_nblocks(N, WyzCfg<NBW>::LG) * WyzCfg<NBW>::YBLK * sizeof(double);
+    return (size_t)wy_nblocks(N, NBW) * WyzCfg<NBW>::YBLK * sizeof(double);
 }
 template <int NBW>
 size_t wyz_scratch_bytes(int64_t N, int64_t nev)
 {
-    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, WyzCfg<NBW>::LG) * sizeof(uint32_t);
+    const size_t prog = (size_t)((nev + 7) >> 3) * (size_t)wy_nchains(N, NBW) * sizeof(uint32_t);
     return wyz_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
@@ -456,7 +456,7 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
         cudaError_t e = set_max_smem((const void *)kern, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
     }
-    const int64_t K0 = wy_nchains(N, C::LG);
+    const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t nslab = (nev + 7) >> 3;
     double *tn_scratch = (double *)scratch;
     uint32_t *prog = (uint32_t *)((char *)scratch + wyz_tn_bytes<NBW>(N));

@@ -17,6 +17,7 @@
 #include "bt_wyz.cuh"
 #include "bc_chase.cuh"
 #include "bt_b2f.cuh"
+#include "bt_b2fz.cuh"
 
 using namespace elpa2bt;
 
@@ -30,11 +31,20 @@ namespace {
 // scratch pool, kernel attributes): no call changes what another thread's or another device's call does
 thread_local int g_variant = 0;
 thread_local int g_last_launches = 0;
+thread_local int g_force_P = 0;     // testing aid (elpa2_bt_set_chain_parallel): warps per slab, 0 = planned
 constexpr int MAX_DEV = 64;
 std::mutex g_mu;        // host-buffer entry point (its cached device scratch)
 std::mutex g_pool_mu;   // creation of the scratch pool
 
-int lg_of(int nbw) { return nbw == 32 ? 5 : nbw == 64 ? 6 : nbw == 128 ? 7 : -1; }
+// Widths (R13, "multiples of 32"): the back-transformation is instantiated for every
+// multiple of 32 up to 256 (real) / 160 (complex: the planar window of one slab must fit in 255
+// registers); the bulge chase and variant 2 for the recommended 32, 64, 128.
+bool bt_width_ok(int nbw, bool cplx) { return nbw >= 32 && (nbw & 31) == 0 && nbw <= (cplx ? 160 : 256); }
+bool pow2_width_ok(int nbw) { return nbw == 32 || nbw == 64 || nbw == 128; }
+
+// expands to `case w: stmt(w)` for the instantiated widths
+#define ELPA2_REAL_WIDTHS(X) X(32) X(64) X(96) X(128) X(160) X(192) X(224) X(256)
+#define ELPA2_CPLX_WIDTHS(X) X(32) X(64) X(96) X(128) X(160)
 
 int current_device()
 {
@@ -135,14 +145,14 @@ cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_
 
 template <int NBW>
 cudaError_t run_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                    cudaStream_t st)
+                    cudaStream_t st, int force_P = 0)
 {
     cudaError_t e;
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
     if ((e = cudaMallocFromPoolAsync(&tn, wyz_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
-    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), tn, st);
+    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), tn, st, force_P);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
@@ -152,9 +162,9 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
         void *stream)
 {
     constexpr int EW = CPLX ? 2 : 1;
-    const int lg = lg_of(nbw);
     if (N < 0) return -1;
-    if (lg < 0) return -2;
+    if (!bt_width_ok(nbw, CPLX)) return -2;
+    if (g_variant == 2 && !pow2_width_ok(nbw)) return -2;
     if (nev < 0) return -3;
     g_last_launches = 0;
     if (N <= 1 || nev == 0) return 0;
@@ -170,23 +180,26 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
     int nlaunch = 1;
     if (g_variant == 1) {
         const unsigned grid = (unsigned)((nev + 127) / 128);
-        bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, lg, nev, hh_v, hh_tau, q, ldq);
+        bt_simple_kernel<CPLX><<<grid, 128, 0, st>>>(N, nbw, nev, hh_v, hh_tau, q, ldq);
         e = cudaGetLastError();
     } else if ((g_variant == 0 || g_variant == 3) && CPLX) {
+        const int fp = g_force_P > 2 ? 2 : g_force_P;
         switch (nbw) {
-        case 32: e = run_wyz<32>(N, nev, hh_v, hh_tau, q, ldq, st); break;
-        case 64: e = run_wyz<64>(N, nev, hh_v, hh_tau, q, ldq, st); break;
-        default: e = run_wyz<128>(N, nev, hh_v, hh_tau, q, ldq, st); break;
+#define X(w) case w: e = run_wyz<w>(N, nev, hh_v, hh_tau, q, ldq, st, fp); break;
+            ELPA2_CPLX_WIDTHS(X)
+#undef X
+        default: return -2;
         }
         nlaunch = 2;
     } else if (g_variant == 0 || (g_variant == 3 && !CPLX)) {
         // variant 3: two chains per pass (pairs of warps share their slabs, hand-over through L2)
         const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
-        const int fp = (g_variant == 3 && wy_nchains(N, lg) >= 8) ? 2 : 0;
+        const int fp = g_force_P ? g_force_P : (g_variant == 3 && wy_nchains(N, nbw) >= 8) ? 2 : 0;
         switch (nbw) {
-        case 32: e = run_wy<32>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
-        case 64: e = run_wy<64>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
-        default: e = run_wy<128>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
+#define X(w) case w: e = run_wy<w>(N, nev, hh_v, hh_tau, q, ldq, align16, st, fp); break;
+            ELPA2_REAL_WIDTHS(X)
+#undef X
+        default: return -2;
         }
         nlaunch = 2;
     } else {
@@ -239,7 +252,7 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
 {
     const size_t esz = is_complex ? 16 : 8;
     if (N < 0) return -1;
-    if (lg_of(nbw) < 0) return -2;
+    if (!bt_width_ok(nbw, is_complex != 0)) return -2;
     if (nev < 0) return -3;
     if (N <= 1 || nev == 0) { g_last_launches = 0; return 0; }
     if (!hh_v) return -4;
@@ -268,7 +281,7 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
                         void *stream)
 {
     if (N < 0) return -1;
-    if (lg_of(nbw) < 0) return -2;
+    if (!pow2_width_ok(nbw)) return -2;
     g_last_launches = 0;
     if (N == 0) return 0;
     if (!ab) return -3;
@@ -312,7 +325,7 @@ int elpa2_bulge_chase_d(int64_t N, int nbw, double *ab, double *hh_v, double *hh
 int elpa2_bulge_chase_z(int64_t N, int nbw, void *ab, void *hh_v, void *hh_tau, double *d, double *e, void *stream)
 {
     if (N < 0) return -1;
-    if (lg_of(nbw) < 0) return -2;
+    if (!pow2_width_ok(nbw)) return -2;
     g_last_launches = 0;
     if (N == 0) return 0;
     if (!ab) return -3;
@@ -380,18 +393,44 @@ int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double 
     return 0;
 }
 
+int elpa2_trans_ev_band_to_full_z(int64_t N, int nbw, int64_t nev, const void *hv, int64_t ldv, const void *tau,
+                                  void *q, int64_t ldq, void *stream)
+{
+    if (N < 0) return -1;
+    if (nbw < 16 || (nbw & 15) != 0) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (N - nbw - 1 <= 0 || nev == 0) return 0;          // no reflector: P = I
+    if (!hv || ((uintptr_t)hv & 15) != 0) return -4;
+    if (ldv < N) return -5;
+    if (!tau || ((uintptr_t)tau & 15) != 0) return -6;
+    if (!q || ((uintptr_t)q & 15) != 0) return -7;
+    if (ldq < N) return -8;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    cudaMemPool_t pool = scratch_pool(&e);
+    if (!pool) return (int)e;
+    void *scratch = nullptr;
+    if ((e = cudaMallocFromPoolAsync(&scratch, b2fz_scratch_bytes(N, nbw), pool, st)) != cudaSuccess) return (int)e;
+    e = launch_b2fz(N, nbw, nev, (const double *)hv, ldv, (const double *)tau, (double *)q, ldq, sm_count(), scratch, st);
+    const cudaError_t e2 = cudaFreeAsync(scratch, st);
+    if (e != cudaSuccess) return (int)e;
+    if (e2 != cudaSuccess) return (int)e2;
+    g_last_launches = 2;
+    return 0;
+}
+
 int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hv, int64_t ldv,
                                      const void *tau, void *q, int64_t ldq)
 {
-    if (is_complex) return -1;                           // complex: device entry point only, for now
-    const size_t esz = 8;
+    const size_t esz = is_complex ? 16 : 8;
     if (N < 0) return -2;
     if (nbw < 16 || (nbw & 15) != 0) return -3;
     if (nev < 0) return -4;
     const int64_t Nv = N - nbw - 1;
     if (Nv <= 0 || nev == 0) { g_last_launches = 0; return 0; }
     if (!hv) return -5;
-    if (ldv < N || (ldv & 1) != 0) return -6;
+    if (ldv < N || (!is_complex && (ldv & 1) != 0)) return -6;
     if (!tau) return -7;
     if (!q) return -8;
     if (ldq < N) return -9;
@@ -404,8 +443,9 @@ int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t
     if ((e = cudaMemcpyAsync(g_sv.p, hv, bv, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
     if ((e = cudaMemcpyAsync(g_st.p, tau, bt, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
     if ((e = cudaMemcpyAsync(g_sq.p, q, bq, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
-    const int rc = elpa2_trans_ev_band_to_full_d(N, nbw, nev, (const double *)g_sv.p, ldv, (const double *)g_st.p,
-                                                 (double *)g_sq.p, ldq, 0);
+    const int rc = is_complex ? elpa2_trans_ev_band_to_full_z(N, nbw, nev, g_sv.p, ldv, g_st.p, g_sq.p, ldq, 0)
+                              : elpa2_trans_ev_band_to_full_d(N, nbw, nev, (const double *)g_sv.p, ldv,
+                                                              (const double *)g_st.p, (double *)g_sq.p, ldq, 0);
     if (rc != 0) return rc < 0 ? rc - 1 : rc;            // argument positions shift by one (is_complex)
     if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
     if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
@@ -414,34 +454,30 @@ int elpa2_trans_ev_band_to_full_host(int is_complex, int64_t N, int nbw, int64_t
 
 int64_t elpa2_hh_count(int64_t N, int nbw)
 {
-    const int lg = lg_of(nbw);
-    if (lg < 0 || N < 2) return 0;
-    return hh_F(N - 1, lg);
+    if (nbw < 1 || N < 2) return 0;
+    return hh_F(N - 1, nbw);
 }
 
 int64_t elpa2_hh_offset(int64_t N, int nbw, int64_t s)
 {
-    const int lg = lg_of(nbw);
-    if (lg < 0 || N < 2 || s < 0 || s > N - 1) return -1;
-    return hh_off(N, lg, s);
+    if (nbw < 1 || N < 2 || s < 0 || s > N - 1) return -1;
+    return hh_off(N, nbw, s);
 }
 
 int elpa2_hh_blocks(int64_t N, int nbw, int64_t s)
 {
-    const int lg = lg_of(nbw);
-    if (lg < 0 || N < 2 || s < 0 || s > N - 2) return 0;
-    return (int)((N - 1 - s + nbw - 1) >> lg);
+    if (nbw < 1 || N < 2 || s < 0 || s > N - 2) return 0;
+    return (int)((N - 1 - s + nbw - 1) / nbw);
 }
 
 int64_t elpa2_hh_lengths(int64_t N, int nbw, int32_t *out, int64_t cap)
 {
-    const int lg = lg_of(nbw);
-    if (lg < 0 || N < 2) return 0;
-    const int64_t G = hh_F(N - 1, lg);
+    if (nbw < 1 || N < 2) return 0;
+    const int64_t G = hh_F(N - 1, nbw);
     if (!out) return G;
     int64_t g = 0;
     for (int64_t s = 0; s <= N - 2; ++s) {
-        const int64_t K = (N - 1 - s + nbw - 1) >> lg;
+        const int64_t K = (N - 1 - s + nbw - 1) / nbw;
         for (int64_t k = 0; k < K; ++k, ++g) {
             if (g >= cap) return G;
             const int64_t rest = N - 1 - s - k * nbw;      // rows r0 .. N-1
@@ -453,21 +489,24 @@ int64_t elpa2_hh_lengths(int64_t N, int nbw, int32_t *out, int64_t cap)
 
 int elpa2_bt_plan(int is_complex, int64_t N, int nbw, int64_t nev, int n_sm, int64_t out[6])
 {
-    const int lg = lg_of(nbw);
     if (N < 0) return -2;
-    if (lg < 0) return -3;
+    if (!bt_width_ok(nbw, is_complex != 0)) return -3;
     if (nev < 0) return -4;
     if (n_sm < 1) return -5;
     if (!out) return -6;
     for (int i = 0; i < 6; ++i) out[i] = 0;
     if (N <= 1 || nev == 0) return 0;
-    const int fp = (g_variant == 3 && !is_complex && wy_nchains(N, lg) >= 8) ? 2 : 0;
+    const int fp = g_force_P ? g_force_P : (g_variant == 3 && !is_complex && wy_nchains(N, nbw) >= 8) ? 2 : 0;
     const WyPlan pl = wy_plan(is_complex != 0, nbw, N, nev, n_sm, fp, is_complex ? 8 : 0);
     size_t scratch = 0;
-    if (is_complex)
-        scratch = nbw == 32 ? wyz_scratch_bytes<32>(N, nev) : nbw == 64 ? wyz_scratch_bytes<64>(N, nev) : wyz_scratch_bytes<128>(N, nev);
-    else
-        scratch = nbw == 32 ? wy_scratch_bytes<32>(N, nev) : nbw == 64 ? wy_scratch_bytes<64>(N, nev) : wy_scratch_bytes<128>(N, nev);
+    switch (nbw + (is_complex ? 1 : 0)) {
+#define X(w) case w: scratch = wy_scratch_bytes<w>(N, nev); break;
+        ELPA2_REAL_WIDTHS(X)
+#undef X
+#define X(w) case w + 1: scratch = wyz_scratch_bytes<w>(N, nev); break;
+        ELPA2_CPLX_WIDTHS(X)
+#undef X
+    }
     out[0] = pl.grid;
     out[1] = pl.nwarps;
     out[2] = pl.P;
@@ -507,6 +546,14 @@ int elpa2_bt_set_variant(int variant)
     if (variant < 0 || variant > 3) return -1;
     const int old = g_variant;
     g_variant = variant;
+    return old;
+}
+
+int elpa2_bt_set_chain_parallel(int P)
+{
+    if (P != 0 && P != 1 && P != 2 && P != 4) return -1;
+    const int old = g_force_P;
+    g_force_P = P;
     return old;
 }
 

@@ -30,7 +30,7 @@ def test_header_symbols_exported(lib):
 
 
 @pytest.mark.parametrize("N", [0, 1, 2, 3, 17, 33, 64, 65, 100, 129, 512, 1000])
-@pytest.mark.parametrize("nbw", [32, 64, 128])
+@pytest.mark.parametrize("nbw", [4, 32, 48, 64, 96, 128, 160, 192, 224, 256])
 def test_layout_helpers_match_oracle(lib, N, nbw):
     assert binding.hh_count(N, nbw) == orc.hh_count(N, nbw)
     for s in range(max(N - 1, 0)):
@@ -42,7 +42,8 @@ def test_layout_helpers_match_oracle(lib, N, nbw):
         assert binding.hh_blocks(N, nbw, N - 1) == 0
 
 
-@pytest.mark.parametrize("N,nbw", [(2, 32), (17, 32), (33, 32), (100, 64), (130, 128), (515, 64), (1000, 32)])
+@pytest.mark.parametrize("N,nbw", [(2, 32), (17, 32), (17, 4), (33, 32), (100, 64), (130, 128), (515, 64), (1000, 32), (700, 96),
+                                   (999, 160), (600, 256)])
 def test_hh_lengths_match_oracle_rows(lib, N, nbw):
     """elpa2_hh_lengths (the only place the binding gets slot lengths from) against the oracle's
     row map, which the paper's worked example pins (tests/test_oracle_layout.py)."""
@@ -83,7 +84,8 @@ def test_layout_full_size_counts(lib):
     assert binding.hh_count(8192, 64) == 528256
     assert binding.hh_count(32768, 64) == 8404480
     assert binding.hh_count(16384, 128) == 1056640
-    assert binding.hh_count(100, 48) == 0          # unsupported nbw
+    assert binding.hh_count(100, 48) == orc.hh_count(100, 48)      # the layout helpers take any nbw >= 1 (R13)
+    assert binding.hh_count(100, 0) == 0
 
 
 def test_argument_validation_codes(lib):
@@ -93,7 +95,8 @@ def test_argument_validation_codes(lib):
     call = binding.trans_ev_tridi_to_band_raw
     for cplx in (False, True):
         assert call(cplx, -1, 64, 4, p16, p16, p16, 8, 0) == -1
-        assert call(cplx, 8, 48, 4, p16, p16, p16, 8, 0) == -2
+        assert call(cplx, 8, 48, 4, p16, p16, p16, 8, 0) == -2        # not a multiple of 32
+        assert call(cplx, 8, 288, 4, p16, p16, p16, 8, 0) == -2       # wider than the widest instantiated kernel
         assert call(cplx, 8, 64, -4, p16, p16, p16, 8, 0) == -3
         assert call(cplx, 8, 64, 4, 0, p16, p16, 8, 0) == -4
         assert call(cplx, 8, 64, 4, p16 + 8, p16, p16, 8, 0) == -4

@@ -64,7 +64,7 @@ def _oracle(N, nbw, hv, tau, x):
     return y
 
 
-@pytest.mark.parametrize("cplx", [False])
+@pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("N,nbw,nev", [(34, 32, 5), (35, 32, 8), (50, 32, 3), (97, 32, 17), (100, 64, 33), (129, 64, 64),
                                        (200, 32, 40), (257, 128, 9), (300, 16, 31), (333, 48, 20), (500, 64, 130)])
 def test_b2f_matches_oracle_on_reduction_output(N, nbw, nev, cplx):
@@ -78,7 +78,7 @@ def test_b2f_matches_oracle_on_reduction_output(N, nbw, nev, cplx):
     assert err <= TOL and err <= _tight(N), (N, nbw, nev, err)
 
 
-@pytest.mark.parametrize("cplx", [False])
+@pytest.mark.parametrize("cplx", [False, True])
 def test_b2f_leading_dimensions_alignment_and_padding(cplx):
     N, nbw, nev = 203, 32, 21
     H = si.dense_hermitian(N, 5, cplx)
@@ -91,30 +91,32 @@ def test_b2f_leading_dimensions_alignment_and_padding(cplx):
         assert np.all(pad == 7.25), (ldq, ldv, off)          # rows >= N of every column untouched
 
 
-def test_b2f_no_work_and_identity_reflectors():
+@pytest.mark.parametrize("cplx", [False, True])
+def test_b2f_no_work_and_identity_reflectors(cplx):
     import torch
 
     from paper_2002_10991_b200 import binding
 
+    dt = np.complex128 if cplx else np.float64
     # Nv = 0 (band as wide as the matrix), nev = 0
     for N, nbw, nev in ((10, 16, 4), (33, 32, 4), (100, 32, 0), (0, 32, 3)):
-        x = _x(N, nev, 1, False)
-        hv = np.zeros((N, max(N - nbw - 1, 0)))
-        got, _ = _run_gpu(N, nbw, hv, np.zeros(hv.shape[1]), x)
+        x = _x(N, nev, 1, cplx)
+        hv = np.zeros((N, max(N - nbw - 1, 0)), dtype=dt)
+        got, _ = _run_gpu(N, nbw, hv, np.zeros(hv.shape[1], dtype=dt), x)
         assert np.array_equal(got, x)
         assert binding.last_launch_count() == 0
     # tau = 0 everywhere: q comes back bit for bit
     N, nbw, nev = 150, 32, 24
     Nv = N - nbw - 1
-    hv = np.zeros((N, Nv))
+    hv = np.zeros((N, Nv), dtype=dt)
     hv[np.arange(Nv) + nbw, np.arange(Nv)] = 1.0
-    x = _x(N, nev, 2, False)
-    got, _ = _run_gpu(N, nbw, hv, np.zeros(Nv), x)
+    x = _x(N, nev, 2, cplx)
+    got, _ = _run_gpu(N, nbw, hv, np.zeros(Nv, dtype=dt), x)
     assert np.array_equal(got, x)
     assert binding.last_launch_count() == 2
 
 
-@pytest.mark.parametrize("cplx", [False])
+@pytest.mark.parametrize("cplx", [False, True])
 def test_b2f_end_to_end_on_device(cplx):
     """6a (oracle) -> 6b, 6d, 6e on the GPU: eigenvectors of the ORIGINAL full matrix."""
     import torch
@@ -142,10 +144,10 @@ def test_b2f_end_to_end_on_device(cplx):
     assert np.abs(C.conj().T @ C - np.eye(N)).max() <= 1e-12 * N
 
 
-@pytest.mark.parametrize("cplx", [False])
+@pytest.mark.parametrize("cplx", [False, True])
 @pytest.mark.parametrize("N,nbw,nev,nsamp", [(1500, 64, 2500, 64), (4096, 64, 20000, 64)])
 def test_b2f_many_slabs_synthetic(N, nbw, nev, nsamp, cplx):
-    """More than one round of 16 slabs per CTA (nev = 20000: 2500 slabs on 148 CTAs), several waves of
+    """More than one round of 16 (complex: 8) slabs per CTA (nev = 20000: 2500 slabs on 148 CTAs), several waves of
     T-factor CTAs; synthetic unitary reflectors; sampled columns + the norm of every column."""
     import torch
 
