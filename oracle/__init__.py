@@ -53,7 +53,7 @@ def lib() -> ctypes.CDLL:
             getattr(_lib, nm).restype = i32
         _lib.orc_tridiag_ql.argtypes = [i64, vp, vp, vp]
         _lib.orc_tridiag_ql.restype = i32
-        for nm in ("orc_back_transform_d", "orc_back_transform_z"):
+        for nm in ("orc_back_transform_d", "orc_back_transform_z", "orc_back_transform_s", "orc_back_transform_c"):
             getattr(_lib, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64]
             getattr(_lib, nm).restype = None
         for nm in ("orc_full_to_band_d", "orc_full_to_band_z"):
@@ -136,14 +136,16 @@ def tridiag_ql(d: np.ndarray, e: np.ndarray):
 def back_transform(N: int, nbw: int, hh_v: np.ndarray, hh_tau: np.ndarray, q: np.ndarray) -> None:
     """q <- H(0,0) ... H(N-2,0) q in place (Eq. 6d), q Fortran-ordered N x ncols."""
     cplx = np.iscomplexobj(q)
-    dt = np.complex128 if cplx else np.float64
-    assert q.dtype == dt and hh_v.dtype == dt and hh_tau.dtype == dt
+    dt = q.dtype
+    assert dt in (np.float64, np.complex128, np.float32, np.complex64)      # FP32: SURVEY 8(f) NEXT-4, reading R16
+    assert hh_v.dtype == dt and hh_tau.dtype == dt
     assert q.ndim == 2 and q.shape[0] == N and q.strides[0] == q.itemsize
     assert hh_v.flags.c_contiguous and hh_tau.flags.c_contiguous
     assert hh_v.shape == (hh_count(N, nbw), nbw)
     ncols = q.shape[1]
     ldq = q.strides[1] // q.itemsize if ncols > 1 else max(N, 1)
-    fn = lib().orc_back_transform_z if cplx else lib().orc_back_transform_d
+    fn = {np.dtype(np.float64): lib().orc_back_transform_d, np.dtype(np.complex128): lib().orc_back_transform_z,
+          np.dtype(np.float32): lib().orc_back_transform_s, np.dtype(np.complex64): lib().orc_back_transform_c}[np.dtype(dt)]
     fn(N, nbw, ncols, _p(hh_v), _p(hh_tau), _p(q), ldq)
 
 

@@ -457,6 +457,84 @@ void orc_back_transform_z(int64_t N, int nbw, int64_t ncols, const zdouble *hh_v
     free(off);
 }
 
+/* ------------------------------------------------------------------------------------------
+ * the same definition (Eq. 8 in reverse generation order) in FP32, real and
+ * complex (R16: the paper runs ELPA in double precision only; single precision is the
+ * library's other build, so the reading is "the same operations with every product and sum rounded
+ * to float").  Inputs are the FP64 reflectors rounded to float by the caller.  ISO C, no FMA
+ * contraction, FLT_EVAL_METHOD 0 on x86-64: each operation is a correctly rounded float operation.
+ * Pins (tests/test_oracle_backtransform.py): agrees with orc_back_transform_d/z on the same rounded
+ * inputs to the FP32 error bound of DESIGN.md "Tolerance (FP32)", preserves column norms to that
+ * bound, and a reversed order misses it by O(1).
+ * ------------------------------------------------------------------------------------------ */
+typedef float _Complex zfloat;
+
+void orc_back_transform_s(int64_t N, int nbw, int64_t ncols, const float *hh_v, const float *hh_tau,
+                          float *q, int64_t ldq)
+{
+    if (N < 2 || ncols < 1) return;
+    int64_t *off = malloc(sizeof(int64_t) * N);
+    off[0] = 0;
+    for (int64_t s = 1; s < N; ++s) off[s] = off[s - 1] + orc_hh_blocks(N, nbw, s - 1);
+    const int64_t chunk = orc_col_chunk(ncols);
+    const int64_t nchunks = (ncols + chunk - 1) / chunk;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t cb = 0; cb < nchunks; ++cb) {
+        int64_t j0 = cb * chunk, j1 = j0 + chunk < ncols ? j0 + chunk : ncols;
+        for (int64_t s = N - 2; s >= 0; --s) {
+            int K = orc_hh_blocks(N, nbw, s);
+            for (int k = 0; k < K; ++k) {
+                int64_t g = off[s] + k, r0, r1;
+                int L = orc_hh_rows(N, nbw, s, k, &r0, &r1);
+                float tau = hh_tau[g];
+                if (tau == 0.0f) continue;
+                const float *v = hh_v + g * nbw;
+                for (int64_t j = j0; j < j1; ++j) {
+                    float *x = q + r0 + j * ldq;
+                    float dot = 0.0f;
+                    for (int r = 0; r < L; ++r) dot += v[r] * x[r];
+                    float td = tau * dot;
+                    for (int r = 0; r < L; ++r) x[r] -= td * v[r];
+                }
+            }
+        }
+    }
+    free(off);
+}
+
+void orc_back_transform_c(int64_t N, int nbw, int64_t ncols, const zfloat *hh_v, const zfloat *hh_tau,
+                          zfloat *q, int64_t ldq)
+{
+    if (N < 2 || ncols < 1) return;
+    int64_t *off = malloc(sizeof(int64_t) * N);
+    off[0] = 0;
+    for (int64_t s = 1; s < N; ++s) off[s] = off[s - 1] + orc_hh_blocks(N, nbw, s - 1);
+    const int64_t chunk = orc_col_chunk(ncols);
+    const int64_t nchunks = (ncols + chunk - 1) / chunk;
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int64_t cb = 0; cb < nchunks; ++cb) {
+        int64_t j0 = cb * chunk, j1 = j0 + chunk < ncols ? j0 + chunk : ncols;
+        for (int64_t s = N - 2; s >= 0; --s) {
+            int K = orc_hh_blocks(N, nbw, s);
+            for (int k = 0; k < K; ++k) {
+                int64_t g = off[s] + k, r0, r1;
+                int L = orc_hh_rows(N, nbw, s, k, &r0, &r1);
+                zfloat tau = hh_tau[g];
+                if (tau == 0.0f) continue;
+                const zfloat *v = hh_v + g * nbw;
+                for (int64_t j = j0; j < j1; ++j) {
+                    zfloat *x = q + r0 + j * ldq;
+                    zfloat dot = 0.0f;
+                    for (int r = 0; r < L; ++r) dot += conjf(v[r]) * x[r];
+                    zfloat td = tau * dot;
+                    for (int r = 0; r < L; ++r) x[r] -= td * v[r];
+                }
+            }
+        }
+    }
+    free(off);
+}
+
 int orc_num_threads(void)
 {
     int n = 1;

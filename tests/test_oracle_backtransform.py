@@ -160,3 +160,41 @@ def test_valid_reorders_are_bit_identical(cplx):
     assert np.abs(Zr - Y).max() <= 1e-14          # same order; rounding of complex mul may differ
     assert np.array_equal(apply(chain_major), Zr)  # bit-identical reorder
     assert np.abs(apply(k_desc) - Zr).max() > 1e-3
+
+
+# ---- FP32 (reading R16): orc_back_transform_{s,c} -------------------------------------
+def tol32(N):
+    """8 u sqrt(N) ||X||_max, u = 2^-24."""
+    return 8.0 * 2.0 ** -24 * np.sqrt(max(N, 1))
+
+
+@pytest.mark.parametrize("cplx", [False, True])
+@pytest.mark.parametrize("N,nbw,ncols", [(17, 4, 12), (64, 32, 20), (300, 32, 9), (700, 64, 5)])
+def test_fp32_back_transform_pinned_to_dense_q2_and_fp64(N, nbw, ncols, cplx):
+    """The FP32 oracle against (a) the dense closed form Q2 X built by numpy in FP64 from the SAME rounded
+    reflectors (tiny N), (b) the FP64 oracle on the same rounded inputs, (c) column norms; (d) the
+    generation-order application misses by O(1)."""
+    _, hh_v, hh_tau, _, _ = _chase(N, nbw, 300 + N, cplx)
+    f32, f64 = (np.complex64, np.complex128) if cplx else (np.float32, np.float64)
+    v32, t32 = hh_v.astype(f32), hh_tau.astype(f32)
+    rng = np.random.default_rng(N)
+    X = (rng.standard_normal((N, ncols)) + (1j * rng.standard_normal((N, ncols)) if cplx else 0)).astype(f32)
+    Y = fortran(X)
+    orc.back_transform(N, nbw, v32, t32, Y)
+    assert Y.dtype == f32
+    xmax = np.abs(X).max()
+    Y64 = fortran(X.astype(f64))
+    orc.back_transform(N, nbw, v32.astype(f64), t32.astype(f64), Y64)
+    assert np.abs(Y - Y64).max() <= tol32(N) * xmax
+    if N <= 64:
+        Q2 = _q2(N, nbw, v32.astype(f64), t32.astype(f64))
+        assert np.abs(Y - Q2 @ X.astype(f64)).max() <= tol32(N) * xmax
+    n0, n1 = np.linalg.norm(X.astype(f64), axis=0), np.linalg.norm(Y.astype(f64), axis=0)
+    assert np.abs(n1 / n0 - 1.0).max() <= tol32(N) * 4
+    # applied in generation order instead (forward over the slots): O(1) away
+    Z = X.astype(f64)
+    for g, s, k, r0, L in _reflector_list(N, nbw):
+        v, t = v32[g, :L].astype(f64), f64(t32[g])
+        Z[r0:r0 + L] -= t * np.outer(v, v.conj() @ Z[r0:r0 + L])
+    if N >= 64:
+        assert np.abs(Z - Y64).max() > 1e-2 * xmax
