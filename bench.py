@@ -50,6 +50,7 @@ CONFIGS = {
 METRIC = "back-transform FP64 GFLOP/s (2N^2*nev real / 8N^2*nev cplx)"
 # FP64 ALU roofline: 148 SMs x 64 DFMA/clk/SM x 2 flop x 1.965 GHz
 NOMINAL_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
+NOMINAL_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 
 
 def source_sha() -> str:
@@ -152,7 +153,7 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_sample_run(cplx, N, nbw, hh_v_np, hh_tau_np, ncols, seed):
+def oracle_sample_run(cplx, N, nbw, hh_v_np, hh_tau_np, ncols, seed, single=False):
     """Times the oracle, as it stands, on ``ncols`` seeded N(0,1) columns.  Returns (seconds, threads)."""
     import numpy as np
 
@@ -162,7 +163,7 @@ def oracle_sample_run(cplx, N, nbw, hh_v_np, hh_tau_np, ncols, seed):
     x = rng.standard_normal((N, ncols))
     if cplx:
         x = x + 1j * rng.standard_normal((N, ncols))
-    x = np.asfortranarray(x)
+    x = np.asfortranarray(x.astype(hh_v_np.dtype) if single else x)
     t0 = time.perf_counter()
     oracle.back_transform(N, nbw, hh_v_np, hh_tau_np, x)
     return time.perf_counter() - t0, oracle.num_threads()
@@ -487,6 +488,9 @@ def main() -> None:
                          "band -> full back-transformation on the same config's N, nbw, nev")
     ap.add_argument("--nev-frac", type=float, default=None,
                     help="partial spectrum (PAPER.md:218): replace nev by round(frac * N)")
+    ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
+                    help="f32: SURVEY 8(f) NEXT-4, the FP32 calls elpa2_trans_ev_tridi_to_band_{s,c} on the config's shape "
+                         "(step 6d only; real nbw <= 128, complex nbw <= 64)")
     ap.add_argument("--shape", default=None, metavar="d|z,N,nbw,nev",
                     help="profiling aid: replace the chosen config's shape (named 'custom' in the output)")
     args = ap.parse_args()
@@ -544,6 +548,13 @@ def main() -> None:
     assert G == binding.hh_count(N, nbw)
     hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
     q = si.gaussian_block(N, nev, seed_x + 7919 * rank, cplx, "cuda")
+    single = args.dtype == "f32"
+    if single:
+        # the FP64 stream rounded to float: unitary to FP32 rounding, same layout
+        f32 = torch.complex64 if cplx else torch.float32
+        hh_v, hh_tau = hh_v.to(f32), hh_tau.to(f32)
+        q = q.t().to(f32).t()                      # keeps the column-major storage
+        esz //= 2
     stream = torch.cuda.current_stream()
     binding.set_variant(args.variant)
 
@@ -618,7 +629,7 @@ def main() -> None:
 
         cores = oracle.num_threads()
         ncols = oracle_sample_cols(cplx, N, cores)
-        tsec, cores = oracle_sample_run(cplx, N, nbw, hh_v.cpu().numpy(), hh_tau.cpu().numpy(), ncols, seed_x)
+        tsec, cores = oracle_sample_run(cplx, N, nbw, hh_v.cpu().numpy(), hh_tau.cpu().numpy(), ncols, seed_x, single)
         cpu = {"value": model_flops(cplx, N, ncols) / tsec / 1e9, "unit": "GFLOP/s", "cores": cores,
                "kind": "oracle", "seconds": tsec,
                "sample": f"{ncols} seeded N(0,1) columns of {nev}, all {G} reflectors "
@@ -628,11 +639,13 @@ def main() -> None:
         kern_ms = sum(step_ms) / len(step_ms)
         achieved = flops / (kern_ms * 1e-3) / 1e12
         traffic, traffic_profile = lookup_traffic("6d", workload_name(args.config)) if args.variant == 0 else (None, None)
+        if single:
+            traffic, traffic_profile = lookup_traffic("6d-f32", workload_name(args.config))
         out = {
             "metric": METRIC, "value": value, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_name(args.config), "N": N, "nbw": nbw, "nev_per_gpu": nev,
+            "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
+            "config": {"workload": workload_name(args.config) + (" [FP32 arithmetic]" if single else ""), "N": N, "nbw": nbw, "nev_per_gpu": nev,
                        "reflector_slots": G,
                        "reflectors": "synthetic unitary stream, device-generated (DESIGN.md input recipe)",
                        "l2": ("inputs larger than L2 (%.2f GiB of q + reflectors per step)"
@@ -654,6 +667,15 @@ def main() -> None:
             "clocks": clk, "e2e": e2e, "gpu_launches": launches, "cpu_baseline": cpu,
             "checks": {"max_rel_column_norm_drift_after_all_steps": norm_dev},
         }
+        if single:
+            # plain FP32 FMA pipe: 148 SMs x 128 FFMA/clk x 2 flop x 1.965 GHz, nominal -- no FP32
+            # figure in MEASURED_PEAKS.json; the metric's model flops are counted in FP32 here
+            out["metric"] = METRIC.replace("FP64", "FP32")
+            out["roofline"] = {"bound": "alu", "achieved": achieved, "peak": NOMINAL_FP32_TFLOPS, "unit": "TFLOP/s",
+                               "frac": achieved / NOMINAL_FP32_TFLOPS,
+                               "peak_source": "nominal FP32 FMA rate: 148 SMs x 128 FFMA/clk x 2 x 1.965 GHz (DESIGN.md 10)",
+                               "kernel": "bt_f32_kernel", "kernel_ms": kern_ms, "algorithmic_flops_per_launch": flops,
+                               "traffic": traffic, "traffic_profile": traffic_profile}
         print(json.dumps(out), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -70,6 +70,21 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
                                       const void *hh_v, const void *hh_tau,
                                       void *q, int64_t ldq);
 
+/* the same operation in FP32 (R16: Eq. 8 with every product and sum in
+ * float; the paper itself runs double precision only).  _s: real float; _c: complex, interleaved (re, im)
+ * floats.  Same layout, same argument positions and error codes as the FP64 calls.  nbw: a multiple of
+ * 32 up to 128 (real) / 64 (complex) -- the window of one column (nbw + 8 rows) sits in the registers of
+ * ONE lane, applied one reflector at a time on the FP32 FMA pipe (there is no FP32 tensor-core type).
+ * hh_v 16-byte aligned; q and hh_tau aligned to their element size (16-byte aligned q with ldq * element
+ * size a multiple of 16 takes the vector path).  One launch, no scratch.  _host32: HOST buffers,
+ * synchronous (is_complex selects _s / _c), as elpa2_trans_ev_tridi_to_band_host. */
+int elpa2_trans_ev_tridi_to_band_s(int64_t N, int nbw, int64_t nev,
+                                   const float *hh_v, const float *hh_tau, float *q, int64_t ldq, void *stream);
+int elpa2_trans_ev_tridi_to_band_c(int64_t N, int nbw, int64_t nev,
+                                   const void *hh_v, const void *hh_tau, void *q, int64_t ldq, void *stream);
+int elpa2_trans_ev_tridi_to_band_host32(int is_complex, int64_t N, int nbw, int64_t nev,
+                                        const void *hh_v, const void *hh_tau, void *q, int64_t ldq);
+
 /* SURVEY.md 8(f) NEXT-1, first version: bulge chasing of a symmetric / Hermitian band matrix to
  * tridiagonal form on the device (Eq. 6b; the step is SURVEY.md 8(c) O3 / DESIGN.md
  * R3, R4, R7), emitting the reflectors in the layout the calls above consume.

@@ -24,6 +24,7 @@ EXPORTS = (
     "elpa2_bulge_chase_d", "elpa2_bulge_chase_z", "elpa2_bt_plan", "elpa2_bt_release_scratch",
     "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z",
     "elpa2_trans_ev_band_to_full_host", "elpa2_bt_set_chain_parallel",
+    "elpa2_trans_ev_tridi_to_band_s", "elpa2_trans_ev_tridi_to_band_c", "elpa2_trans_ev_tridi_to_band_host32",
 )
 
 
@@ -48,9 +49,12 @@ def lib() -> ctypes.CDLL:
                 "(there is no CPU fallback)")
         L = ctypes.CDLL(LIB_PATH)
         i64, i32, vp = ctypes.c_int64, ctypes.c_int, ctypes.c_void_p
-        for nm in ("elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z"):
+        for nm in ("elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z",
+                   "elpa2_trans_ev_tridi_to_band_s", "elpa2_trans_ev_tridi_to_band_c"):
             getattr(L, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64, vp]
             getattr(L, nm).restype = i32
+        L.elpa2_trans_ev_tridi_to_band_host32.argtypes = [i32, i64, i32, i64, vp, vp, vp, i64]
+        L.elpa2_trans_ev_tridi_to_band_host32.restype = i32
         L.elpa2_trans_ev_tridi_to_band_host.argtypes = [i32, i64, i32, i64, vp, vp, vp, i64]
         L.elpa2_trans_ev_tridi_to_band_host.restype = i32
         for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
@@ -169,23 +173,28 @@ def _stream_ptr(stream) -> int:
 
 
 def trans_ev_tridi_to_band_raw(cplx: bool, N: int, nbw: int, nev: int, hh_v_ptr: int, hh_tau_ptr: int,
-                               q_ptr: int, ldq: int, stream_ptr: int) -> int:
-    """The C call itself, on raw device addresses; returns the C return code."""
-    fn = lib().elpa2_trans_ev_tridi_to_band_z if cplx else lib().elpa2_trans_ev_tridi_to_band_d
+                               q_ptr: int, ldq: int, stream_ptr: int, single: bool = False) -> int:
+    """The C call itself, on raw device addresses; returns the C return code.  ``single``: the FP32 calls."""
+    if single:
+        fn = lib().elpa2_trans_ev_tridi_to_band_c if cplx else lib().elpa2_trans_ev_tridi_to_band_s
+    else:
+        fn = lib().elpa2_trans_ev_tridi_to_band_z if cplx else lib().elpa2_trans_ev_tridi_to_band_d
     return fn(N, nbw, nev, hh_v_ptr, hh_tau_ptr, q_ptr, ldq, stream_ptr)
 
 
 def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> None:
-    """q <- Q2 q in place (Eq. 6d).  ``q``: CUDA tensor of shape (N, nev), float64 or complex128,
-    stored column-major (``q.stride(0) == 1``; ldq = ``q.stride(1)``).  ``hh_v`` (G, nbw) and
+    """q <- Q2 q in place (Eq. 6d).  ``q``: CUDA tensor of shape (N, nev), float64 or complex128 (or
+    float32 / complex64: the FP32 calls), stored column-major (``q.stride(0) == 1``; ldq = ``q.stride(1)``).  ``hh_v`` (G, nbw) and
     ``hh_tau`` (G,) contiguous CUDA tensors of the same dtype, layout per include/elpa2_bt.h."""
     import torch
 
     if not (q.is_cuda and hh_v.is_cuda and hh_tau.is_cuda):
         raise ValueError("device tensors required (use trans_ev_tridi_to_band_host for numpy arrays)")
-    cplx = q.dtype == torch.complex128
-    if q.dtype not in (torch.float64, torch.complex128) or hh_v.dtype != q.dtype or hh_tau.dtype != q.dtype:
-        raise ValueError("float64 or complex128 throughout")
+    cplx = q.dtype in (torch.complex128, torch.complex64)
+    single = q.dtype in (torch.float32, torch.complex64)
+    if (q.dtype not in (torch.float64, torch.complex128, torch.float32, torch.complex64) or hh_v.dtype != q.dtype
+            or hh_tau.dtype != q.dtype):
+        raise ValueError("one of float64, complex128, float32, complex64 throughout")
     if q.dim() != 2 or q.shape[0] != N or (q.shape[0] > 1 and q.stride(0) != 1):
         raise ValueError("q must be (N, nev) column-major")
     nev = q.shape[1]
@@ -200,7 +209,7 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
     if torch.cuda.current_device() != q.device.index:
         raise ValueError("q's device must be the current CUDA device")
     rc = trans_ev_tridi_to_band_raw(cplx, N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q.data_ptr(),
-                                    ldq, _stream_ptr(stream))
+                                    ldq, _stream_ptr(stream), single)
     if rc != 0:
         raise Elpa2BtError(rc)
 
@@ -278,16 +287,17 @@ def trans_ev_tridi_to_band_host(N: int, nbw: int, hh_v, hh_tau, q) -> None:
     import numpy as np
 
     cplx = np.iscomplexobj(q)
-    dt = np.complex128 if cplx else np.float64
-    if q.dtype != dt or hh_v.dtype != dt or hh_tau.dtype != dt:
-        raise ValueError("float64 or complex128 throughout")
+    dt = q.dtype
+    if dt not in (np.float64, np.complex128, np.float32, np.complex64) or hh_v.dtype != dt or hh_tau.dtype != dt:
+        raise ValueError("one of float64, complex128, float32, complex64 throughout")
+    single = dt in (np.float32, np.complex64)
     if q.ndim != 2 or q.shape[0] != N or (N > 1 and q.strides[0] != q.itemsize):
         raise ValueError("q must be (N, nev) column-major")
     nev = q.shape[1]
     ldq = q.strides[1] // q.itemsize if nev > 1 else max(N, 1)
     if nev > 1 and not q.flags.f_contiguous:
         raise ValueError("host q must be Fortran-contiguous (ldq == N)")
-    rc = lib().elpa2_trans_ev_tridi_to_band_host(int(cplx), N, nbw, nev, hh_v.ctypes.data, hh_tau.ctypes.data,
-                                                 q.ctypes.data, ldq)
+    fn = lib().elpa2_trans_ev_tridi_to_band_host32 if single else lib().elpa2_trans_ev_tridi_to_band_host
+    rc = fn(int(cplx), N, nbw, nev, hh_v.ctypes.data, hh_tau.ctypes.data, q.ctypes.data, ldq)
     if rc != 0:
         raise Elpa2BtError(rc)

@@ -18,6 +18,7 @@
 #include "bc_chase.cuh"
 #include "bt_b2f.cuh"
 #include "bt_b2fz.cuh"
+#include "bt_f32.cuh"
 
 using namespace elpa2bt;
 
@@ -45,6 +46,8 @@ bool pow2_width_ok(int nbw) { return nbw == 32 || nbw == 64 || nbw == 128; }
 // expands to `case w: stmt(w)` for the instantiated widths
 #define ELPA2_REAL_WIDTHS(X) X(32) X(64) X(96) X(128) X(160) X(192) X(224) X(256)
 #define ELPA2_CPLX_WIDTHS(X) X(32) X(64) X(96) X(128) X(160)
+// FP32 (bt_f32.cuh): the window of one column sits in one lane's registers
+bool f32_width_ok(int nbw, bool cplx) { return nbw >= 32 && (nbw & 31) == 0 && nbw <= (cplx ? 64 : 128); }
 
 int current_device()
 {
@@ -215,6 +218,33 @@ int run(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_ta
     return 0;
 }
 
+template <bool CPLX>
+int run_f32(int64_t N, int nbw, int64_t nev, const float *hh_v, const float *hh_tau, float *q, int64_t ldq, void *stream)
+{
+    constexpr int EW = CPLX ? 2 : 1;
+    if (N < 0) return -1;
+    if (!f32_width_ok(nbw, CPLX)) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (N <= 1 || nev == 0) return 0;
+    if (!hh_v || ((uintptr_t)hh_v & 15) != 0) return -4;
+    if (!hh_tau || ((uintptr_t)hh_tau & (4 * EW - 1)) != 0) return -5;
+    if (!q || ((uintptr_t)q & (4 * EW - 1)) != 0) return -6;
+    if (ldq < N) return -7;
+    const int align16 = (((uintptr_t)q & 15) == 0 && ((ldq * EW) & 3) == 0) ? 1 : 0;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    switch (nbw) {
+    case 32: e = launch_f32<CPLX, 32>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), st); break;
+    case 64: e = launch_f32<CPLX, 64>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), st); break;
+    case 96: e = launch_f32<false, 96>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), st); break;
+    default: e = launch_f32<false, 128>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), st); break;
+    }
+    if (e != cudaSuccess) return (int)e;
+    g_last_launches = 1;
+    return 0;
+}
+
 // grow-only device scratch for the host-buffer entry point
 struct Scratch {
     void *p = nullptr;
@@ -245,6 +275,48 @@ int elpa2_trans_ev_tridi_to_band_z(int64_t N, int nbw, int64_t nev, const void *
                                    void *q, int64_t ldq, void *stream)
 {
     return run<true>(N, nbw, nev, (const double *)hh_v, (const double *)hh_tau, (double *)q, ldq, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_s(int64_t N, int nbw, int64_t nev, const float *hh_v, const float *hh_tau,
+                                   float *q, int64_t ldq, void *stream)
+{
+    return run_f32<false>(N, nbw, nev, hh_v, hh_tau, q, ldq, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_c(int64_t N, int nbw, int64_t nev, const void *hh_v, const void *hh_tau,
+                                   void *q, int64_t ldq, void *stream)
+{
+    return run_f32<true>(N, nbw, nev, (const float *)hh_v, (const float *)hh_tau, (float *)q, ldq, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_host32(int is_complex, int64_t N, int nbw, int64_t nev, const void *hh_v,
+                                        const void *hh_tau, void *q, int64_t ldq)
+{
+    const size_t esz = is_complex ? 8 : 4;
+    if (N < 0) return -1;
+    if (!f32_width_ok(nbw, is_complex != 0)) return -2;
+    if (nev < 0) return -3;
+    if (N <= 1 || nev == 0) { g_last_launches = 0; return 0; }
+    if (!hh_v) return -4;
+    if (!hh_tau) return -5;
+    if (!q) return -6;
+    if (ldq < N) return -7;
+    std::lock_guard<std::mutex> lock(g_mu);
+    const size_t G = (size_t)elpa2_hh_count(N, nbw);
+    const size_t bv = G * nbw * esz, bt = G * esz, bq = (size_t)ldq * nev * esz;
+    cudaError_t e;
+    if ((e = g_sv.reserve(bv)) != cudaSuccess) return (int)e;
+    if ((e = g_st.reserve(bt)) != cudaSuccess) return (int)e;
+    if ((e = g_sq.reserve(bq)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sv.p, hh_v, bv, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_st.p, hh_tau, bt, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaMemcpyAsync(g_sq.p, q, bq, cudaMemcpyHostToDevice, 0)) != cudaSuccess) return (int)e;
+    int rc = is_complex ? run_f32<true>(N, nbw, nev, (const float *)g_sv.p, (const float *)g_st.p, (float *)g_sq.p, ldq, 0)
+                        : run_f32<false>(N, nbw, nev, (const float *)g_sv.p, (const float *)g_st.p, (float *)g_sq.p, ldq, 0);
+    if (rc != 0) return rc;
+    if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
+    if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
+    return 0;
 }
 
 int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hh_v,
