@@ -70,6 +70,28 @@ int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_
                                       const void *hh_v, const void *hh_tau,
                                       void *q, int64_t ldq);
 
+/* the row-block form of the same operation -- the building block of the row-pipelined
+ * multi-GPU variant (an eigenvector's rows spread over a process column, "at most nbw"
+ * rows exchanged with the neighbour per step).  The caller owns the rows
+ * [row0, row0 + nown) of q (row0 a multiple of 8; nown a multiple of 8 unless the block ends at row N)
+ * and passes q_local, which holds the rows [row0, row0 + nloc) of its columns, nloc >= min(nown + nbw,
+ * N - row0): the owned rows followed by the <= nbw halo rows of the neighbour below (larger row
+ * indices), leading dimension ldq >= nloc.  For the chains k = kb .. ke-1 in order (chain k = the
+ * reflectors (s, k) of all sweeps, applied s descending: the chain-major order of R5) the call applies the
+ * reflectors whose FIRST row lies in the owned rows (in units of 8-row blocks), reading and updating the halo
+ * rows they reach into.  Applying, for every chain in turn, the row blocks from the bottom of the matrix
+ * to the top -- each with the halo rows as its lower neighbour left them, and handing its own first nbw
+ * rows on as the upper neighbour's halo -- is the whole back-transformation, bit for bit the result of
+ * elpa2_trans_ev_tridi_to_band_{d,z} (the same kernels run a sub-range of their block sequence).
+ * Argument positions: N=1, nbw=2, nev=3, hh_v=4, hh_tau=5, q_local=6, ldq=7, row0=8, nown=9, nloc=10,
+ * kb/ke=11; > 0 = cudaError_t.  Asynchronous on `stream`; scratch for the chains [kb, ke) only. */
+int elpa2_trans_ev_tridi_to_band_rows_d(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau,
+                                        double *q_local, int64_t ldq, int64_t row0, int64_t nown, int64_t nloc,
+                                        int64_t kb, int64_t ke, void *stream);
+int elpa2_trans_ev_tridi_to_band_rows_z(int64_t N, int nbw, int64_t nev, const void *hh_v, const void *hh_tau,
+                                        void *q_local, int64_t ldq, int64_t row0, int64_t nown, int64_t nloc,
+                                        int64_t kb, int64_t ke, void *stream);
+
 /* the same operation in FP32 (R16: Eq. 8 with every product and sum in
  * float; the paper itself runs double precision only).  _s: real float; _c: complex, interleaved (re, im)
  * floats.  Same layout, same argument positions and error codes as the FP64 calls.  nbw: a multiple of

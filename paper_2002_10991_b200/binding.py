@@ -25,6 +25,7 @@ EXPORTS = (
     "elpa2_hh_lengths", "elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z",
     "elpa2_trans_ev_band_to_full_host", "elpa2_bt_set_chain_parallel",
     "elpa2_trans_ev_tridi_to_band_s", "elpa2_trans_ev_tridi_to_band_c", "elpa2_trans_ev_tridi_to_band_host32",
+    "elpa2_trans_ev_tridi_to_band_rows_d", "elpa2_trans_ev_tridi_to_band_rows_z",
 )
 
 
@@ -52,6 +53,9 @@ def lib() -> ctypes.CDLL:
         for nm in ("elpa2_trans_ev_tridi_to_band_d", "elpa2_trans_ev_tridi_to_band_z",
                    "elpa2_trans_ev_tridi_to_band_s", "elpa2_trans_ev_tridi_to_band_c"):
             getattr(L, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64, vp]
+            getattr(L, nm).restype = i32
+        for nm in ("elpa2_trans_ev_tridi_to_band_rows_d", "elpa2_trans_ev_tridi_to_band_rows_z"):
+            getattr(L, nm).argtypes = [i64, i32, i64, vp, vp, vp, i64, i64, i64, i64, i64, i64, vp]
             getattr(L, nm).restype = i32
         L.elpa2_trans_ev_tridi_to_band_host32.argtypes = [i32, i64, i32, i64, vp, vp, vp, i64]
         L.elpa2_trans_ev_tridi_to_band_host32.restype = i32
@@ -210,6 +214,35 @@ def trans_ev_tridi_to_band(N: int, nbw: int, hh_v, hh_tau, q, stream=None) -> No
         raise ValueError("q's device must be the current CUDA device")
     rc = trans_ev_tridi_to_band_raw(cplx, N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q.data_ptr(),
                                     ldq, _stream_ptr(stream), single)
+    if rc != 0:
+        raise Elpa2BtError(rc)
+
+
+def trans_ev_tridi_to_band_rows(N: int, nbw: int, hh_v, hh_tau, q_local, row0: int, nown: int, kb: int, ke: int,
+                                stream=None) -> None:
+    """Row-block form (include/elpa2_bt.h): ``q_local`` is a column-major CUDA tensor of
+    shape (nloc, nev) holding the rows [row0, row0 + nloc) -- the ``nown`` owned rows and the halo rows
+    below; applies the owned blocks of the chains [kb, ke)."""
+    import torch
+
+    if not (q_local.is_cuda and hh_v.is_cuda and hh_tau.is_cuda):
+        raise ValueError("device tensors required")
+    cplx = q_local.dtype == torch.complex128
+    if q_local.dtype not in (torch.float64, torch.complex128) or hh_v.dtype != q_local.dtype or hh_tau.dtype != q_local.dtype:
+        raise ValueError("float64 or complex128 throughout")
+    if q_local.dim() != 2 or (q_local.shape[0] > 1 and q_local.stride(0) != 1):
+        raise ValueError("q_local must be (nloc, nev) column-major")
+    nloc, nev = q_local.shape
+    ldq = q_local.stride(1) if nev > 1 else max(nloc, 1)
+    G = hh_count(N, nbw)
+    if not (hh_v.is_contiguous() and hh_tau.is_contiguous()) or tuple(hh_v.shape) != (G, nbw) or tuple(hh_tau.shape) != (G,):
+        raise ValueError(f"hh_v must be contiguous ({G}, {nbw}) and hh_tau ({G},)")
+    if not (hh_v.device == q_local.device and hh_tau.device == q_local.device
+            and torch.cuda.current_device() == q_local.device.index):
+        raise ValueError("hh_v, hh_tau and q_local must live on the current CUDA device")
+    fn = lib().elpa2_trans_ev_tridi_to_band_rows_z if cplx else lib().elpa2_trans_ev_tridi_to_band_rows_d
+    rc = fn(N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q_local.data_ptr(), ldq, row0, nown, nloc, kb, ke,
+            _stream_ptr(stream))
     if rc != 0:
         raise Elpa2BtError(rc)
 

@@ -68,6 +68,11 @@ struct WyArgs {
     uint32_t *prog;        // chain-parallel mode: prog[slab * K0 + k] = blocks of chain k finished (zeroed per call)
     int align16;           // q base and ldq*8 are 16-byte aligned
     int P;                 // warps per slab (1, 2 or 4), each on its own chains k = p, p+P, ...
+    // Sub-range launches (rowpipe: a rank that owns a block of rows): chains [kb, ke),
+    // of each chain only the blocks b_bot <= b <= b_top; rows >= row_end are not in memory (read as zero,
+    // never written); q and tn are pre-shifted so that global row / block indices address them.  The whole
+    // matrix is kb = 0, ke = K0, b_top = bhi, b_bot = 0, row_end = N.
+    int64_t kb, ke, b_top, b_bot, row_end;
 };
 
 // ---- block enumeration ----------------------------------------------------------------------------
@@ -114,7 +119,7 @@ __device__ __forceinline__ void cp_async_mbar_arrive_noinc_wy(uint32_t bar)
 template <int NBW>
 __global__ void __launch_bounds__(WyCfg<NBW>::PW * 32) wy_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
                                                                          const double *__restrict__ hh_tau,
-                                                                         double *__restrict__ yb)
+                                                                         double *__restrict__ yb, int64_t kb)
 {
     using C = WyCfg<NBW>;
     constexpr int W = C::W, SV = W + 2;               // Vs row stride: rows r, r+1 land 4 banks apart
@@ -122,7 +127,7 @@ __global__ void __launch_bounds__(WyCfg<NBW>::PW * 32) wy_prepass_kernel(int64_t
     __shared__ double Vs[C::PW][8 * SV];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gq = lane >> 2, r = lane & 3;
-    const int64_t k = blockIdx.y;
+    const int64_t k = kb + blockIdx.y;
     const int64_t bhi = wy_bhi(N);
     const int64_t nblk = bhi - (k * C::NB8) + 1;
     const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
@@ -224,25 +229,25 @@ __device__ __forceinline__ void wy_load2(const WyArgs &a, const double *colp, bo
 {
     x0 = 0.0;
     x1 = 0.0;
-    if (!colok || row >= a.N) return;
-    if (a.align16 && row + 1 < a.N) {
+    if (!colok || row >= a.row_end) return;
+    if (a.align16 && row + 1 < a.row_end) {
         const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + row))
                              : *reinterpret_cast<const double2 *>(colp + row);
         x0 = v.x;
         x1 = v.y;
     } else {
         x0 = CG ? __ldcg(colp + row) : colp[row];
-        if (row + 1 < a.N) x1 = CG ? __ldcg(colp + row + 1) : colp[row + 1];
+        if (row + 1 < a.row_end) x1 = CG ? __ldcg(colp + row + 1) : colp[row + 1];
     }
 }
 __device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double x0, double x1)
 {
-    if (!colok || row >= a.N) return;
-    if (a.align16 && row + 1 < a.N) {
+    if (!colok || row >= a.row_end) return;
+    if (a.align16 && row + 1 < a.row_end) {
         *reinterpret_cast<double2 *>(colp + row) = make_double2(x0, x1);
     } else {
         colp[row] = x0;
-        if (row + 1 < a.N) colp[row + 1] = x1;
+        if (row + 1 < a.row_end) colp[row + 1] = x1;
     }
 }
 
@@ -265,7 +270,8 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::NBW);
-    const int64_t bhi = wy_bhi(N);
+    const int64_t bhi = wy_bhi(N);                      // numbering of the blocks (scratch ids) is global
+    const int64_t btop = a.b_top;                       // first block of every chain in this launch (bhi: whole matrix)
     const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1
@@ -277,13 +283,14 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const bool fastio = a.align16 && (col0 + 8 * NG <= a.nev);
 
     // staging cursor: block it + NSP - LAG of this ring's sequence
-    int64_t pk = grp, pb = bhi;
+    auto bbot = [&](int64_t k) { return k * C::NB8 > a.b_bot ? k * C::NB8 : a.b_bot; };   // last block of chain k here
+    int64_t pk = a.kb + grp, pb = btop;
     auto advance = [&]() {
-        if (pb > (pk * C::NB8)) {
+        if (pb > bbot(pk)) {
             --pb;
         } else {
             pk += P;
-            pb = bhi;
+            pb = btop;
         }
     };
     auto stage_cursor = [&](uint32_t st) {
@@ -292,7 +299,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     };
     // prologue: blocks 0 .. NSP-LAG-1 go into fresh stages
     for (int i = 0; i < NSP - LAG; ++i) {
-        if (member == 0 && pk < K0) stage_cursor((uint32_t)i);
+        if (member == 0 && pk < a.ke) stage_cursor((uint32_t)i);
         advance();
     }
 
@@ -306,15 +313,15 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     double X[NG][NT + 1][2], TA[NG][2], TB[NG][2];
     uint32_t it = 0;                   // blocks consumed from this ring
     int duty = 0;
-    for (int64_t k = grp; k < K0; k += P) {
-        const int64_t blo = k * C::NB8;
+    for (int64_t k = a.kb + grp; k < a.ke; k += P) {
+        const int64_t blo = bbot(k);
         // chain-parallel hand-over: chain k-1 of this slab is walked by another warp of the CTA
-        const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
+        const uint32_t *prev = (CP && k > a.kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
         uint32_t known = 0;
         auto wait_prev = [&](int64_t b) {          // before loading tile 0 of block b
             if (CP && prev) {
-                const uint32_t need = (uint32_t)(bhi - b + NBW / 8 + 1);
+                const uint32_t need = (uint32_t)(btop - b + NBW / 8 + 1);
                 while (known < need) known = prog_read(prev);
             }
         };
@@ -330,7 +337,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             // --- staging duty: block it+NSP-LAG goes into the stage that block it-LAG used; the warp
             //     on duty only waits if some member is still LAG blocks behind it
             if (duty == member) {
-                if (pk < K0) {
+                if (pk < a.ke) {
                     const uint32_t st = (it + NSP - LAG) & (NSP - 1);
                     if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
                     stage_cursor(st);
@@ -390,11 +397,11 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
                 mbar_arrive(bar_empty + 8 * st);
                 // the stores of the blocks before this one have long been performed: publishing them
                 // here keeps the release fence off the critical path (costs one block of extra lag)
-                if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
+                if (CP && b < btop) prog_publish(mine, (uint32_t)(btop - b));
             }
             // --- tile NT-1 retires (rows 8b + nbw ..), the buffer of tile 0 is refilled
             const int64_t bn = b - (PF2 ? 2 : 1);
-            if (fastio && (b << 3) + NBW + 8 <= N) {
+            if (fastio && (b << 3) + NBW + 8 <= a.row_end) {
                 double *pr = cb + (b << 3) + 2 * r;
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
@@ -419,21 +426,26 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             ++it;
         };
 
+        // the window above tile 0: rows 8 btop + 8t ..; beyond the matrix (the whole-matrix launch: every
+        // one of them) they read as zero without touching memory, in a sub-range launch they are the rows
+        // the rank below handed over
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
 #pragma unroll
-            for (int t = 1; t <= NT; ++t) X[g][t][0] = X[g][t][1] = 0.0;
+            for (int t = 1; t < NT; ++t)
+                wy_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, X[g][t][0], X[g][t][1]);
+            X[g][NT][0] = X[g][NT][1] = 0.0;
             TA[g][0] = TA[g][1] = TB[g][0] = TB[g][1] = 0.0;
         }
-        load_tile0(bhi, TA);
+        load_tile0(btop, TA);
         if (PF2) {
-            load_tile0(bhi - 1, TB);
-            for (int64_t b = bhi; b >= blo; b -= 2) {
+            load_tile0(btop - 1, TB);
+            for (int64_t b = btop; b >= blo; b -= 2) {
                 do_block(b, TA);
                 if (b - 1 >= blo) do_block(b - 1, TB);
             }
         } else {
-            for (int64_t b = bhi; b >= blo; --b) do_block(b, TA);
+            for (int64_t b = btop; b >= blo; --b) do_block(b, TA);
         }
         // --- chain end: tiles 1 .. NT-1 hold rows 8 blo + 8 (t-1) + 2r + {0,1}
 #pragma unroll
@@ -443,7 +455,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
                 wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
         if (CP) {
             __syncwarp();
-            if (lane == 0) prog_publish(mine, (uint32_t)(bhi - blo + 1));
+            if (lane == 0) prog_publish(mine, (uint32_t)(btop - blo + 1));
         }
     }
 }
@@ -582,17 +594,56 @@ cudaError_t launch_wy_main(const WyArgs &a, const WyPlan &pl, cudaStream_t st)
     return cudaGetLastError();
 }
 
+// Sub-range of a launch: the chains [kb, ke) restricted to the blocks whose first row
+// lies in the rows [row0, row0 + nown) this caller owns; its q holds the rows [row0, row_end).  row0 a
+// multiple of 8.  The whole matrix: kb = 0, ke = -1 (= K0), row0 = 0, nown = row_end = N.
+struct WyRange {
+    int64_t kb = 0, ke = -1, row0 = 0, nown = -1, row_end = -1;
+    bool whole() const { return ke < 0; }
+};
+// chains of the range that have a block here, block bounds (host arithmetic shared by real and complex)
+inline void wy_range_resolve(const WyRange &r, int64_t N, int nbw, int64_t &kb, int64_t &ke, int64_t &b_top, int64_t &b_bot,
+                             int64_t &row_end)
+{
+    const int64_t K0 = wy_nchains(N, nbw), bhi = wy_bhi(N);
+    if (r.whole()) {
+        kb = 0, ke = K0, b_top = bhi, b_bot = 0, row_end = N;
+        return;
+    }
+    b_bot = r.row0 >> 3;
+    b_top = ((r.row0 + r.nown) >> 3) - 1;
+    if (r.row0 + r.nown >= N || b_top > bhi) b_top = bhi;
+    row_end = r.row_end;
+    kb = r.kb;
+    ke = r.ke < K0 ? r.ke : K0;
+    const int64_t klast = b_top / (nbw >> 3);          // chains beyond it start below this range
+    if (ke > klast + 1) ke = klast + 1;
+    if (ke < kb) ke = kb;
+}
+template <int NBW>
+size_t wy_tn_bytes_range(int64_t N, int64_t kb, int64_t ke)
+{
+    return (size_t)(wy_base(N, NBW, ke) - wy_base(N, NBW, kb)) * WyCfg<NBW>::YBLK * sizeof(double);
+}
+
 // force_P > 0 overrides the number of warps per slab of the 8-warp kernel; force_nw = 8 keeps the
 // 16-warp kernel (few columns: 4 warps per slab, 128 registers each) from being chosen.
+// A sub-range launch (rg) runs P = 1 on the 8-warp kernel; `scratch` then holds the chains [kb, ke) only.
 template <int NBW>
 cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                      int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0, int force_nw = 0)
+                      int align16, int nsm, void *scratch, cudaStream_t st, int force_P = 0, int force_nw = 0,
+                      const WyRange &rg = WyRange())
 {
     using C = WyCfg<NBW>;
     const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t nslab = (nev + 7) >> 3;
-    double *tn = (double *)scratch;
-    uint32_t *prog = (uint32_t *)((char *)scratch + wy_tn_bytes<NBW>(N));
+    WyArgs a;
+    wy_range_resolve(rg, N, NBW, a.kb, a.ke, a.b_top, a.b_bot, a.row_end);
+    if (a.ke <= a.kb) return cudaSuccess;
+    if (!rg.whole()) force_P = 1, force_nw = 8;
+    const size_t tn_bytes = rg.whole() ? wy_tn_bytes<NBW>(N) : wy_tn_bytes_range<NBW>(N, a.kb, a.ke);
+    double *tn = (double *)scratch - wy_base(N, NBW, a.kb) * C::YBLK;      // addressed by global block ids
+    uint32_t *prog = (uint32_t *)((char *)scratch + tn_bytes);
     const WyPlan pl = wy_plan(false, NBW, N, nev, nsm, force_P, force_nw);
     const int P = pl.P;
     cudaError_t e;
@@ -600,17 +651,16 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
     }
-    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)K0);
-    wy_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)(a.ke - a.kb));
+    wy_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn, a.kb);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    WyArgs a;
     a.N = N;
     a.nev = nev;
     a.ldq = ldq;
     a.hh_v = hh_v;
     a.hh_tau = hh_tau;
-    a.q = q;
+    a.q = q - rg.row0;                                  // addressed by global row indices
     a.tn = tn;
     a.prog = prog;
     a.align16 = align16;

@@ -45,7 +45,7 @@ struct WyzCfg {
 template <int NBW>
 __global__ void __launch_bounds__(WyzCfg<NBW>::PW * 32) wyz_prepass_kernel(int64_t N, const double *__restrict__ hh_v,
                                                                            const double *__restrict__ hh_tau,
-                                                                           double *__restrict__ yb)
+                                                                           double *__restrict__ yb, int64_t kb)
 {
     using C = WyzCfg<NBW>;
     constexpr int W = C::W, SV = W + 1;               // Vs row stride (elements)
@@ -53,7 +53,7 @@ __global__ void __launch_bounds__(WyzCfg<NBW>::PW * 32) wyz_prepass_kernel(int64
     __shared__ double Vs[C::PW][8 * SV * 2];
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int gq = lane >> 2, r = lane & 3;
-    const int64_t k = blockIdx.y;
+    const int64_t k = kb + blockIdx.y;
     const int64_t bhi = wy_bhi(N);
     const int64_t nblk = bhi - (k * C::NB8) + 1;
     const int64_t j = (int64_t)blockIdx.x * C::PW + warp;
@@ -173,12 +173,12 @@ __device__ __forceinline__ void wyz_load2(const WyArgs &a, const double *colp, b
                                           double &xr1, double &xi0, double &xi1)
 {
     xr0 = xr1 = xi0 = xi1 = 0.0;
-    if (!colok || row >= a.N) return;
+    if (!colok || row >= a.row_end) return;
     const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row))
                          : *reinterpret_cast<const double2 *>(colp + 2 * row);
     xr0 = v.x;
     xi0 = v.y;
-    if (row + 1 < a.N) {
+    if (row + 1 < a.row_end) {
         const double2 w = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row + 2))
                              : *reinterpret_cast<const double2 *>(colp + 2 * row + 2);
         xr1 = w.x;
@@ -188,9 +188,9 @@ __device__ __forceinline__ void wyz_load2(const WyArgs &a, const double *colp, b
 __device__ __forceinline__ void wyz_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double xr0,
                                            double xr1, double xi0, double xi1)
 {
-    if (!colok || row >= a.N) return;
+    if (!colok || row >= a.row_end) return;
     *reinterpret_cast<double2 *>(colp + 2 * row) = make_double2(xr0, xi0);
-    if (row + 1 < a.N) *reinterpret_cast<double2 *>(colp + 2 * row + 2) = make_double2(xr1, xi1);
+    if (row + 1 < a.row_end) *reinterpret_cast<double2 *>(colp + 2 * row + 2) = make_double2(xr1, xi1);
 }
 
 // ---- a warp with NG slabs of 8 columns -------------------------------------------------------------------
@@ -209,7 +209,8 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     const int gq = lane >> 2, r = lane & 3;
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::NBW);
-    const int64_t bhi = wy_bhi(N);
+    const int64_t bhi = wy_bhi(N);                      // numbering of the blocks (scratch ids) is global
+    const int64_t btop = a.b_top;                       // first block of every chain in this launch (bt_wy.cuh)
     const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1 (ldq counts complex elements)
@@ -218,13 +219,14 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
     const bool fastio = col0 + 8 * NG <= a.nev;         // warp-uniform: every column of the warp exists
 
-    int64_t pk = grp, pb = bhi;                         // staging cursor: block it + NSP - LAG of this ring
+    auto bbot = [&](int64_t k) { return k * C::NB8 > a.b_bot ? k * C::NB8 : a.b_bot; };   // last block of chain k here
+    int64_t pk = a.kb + grp, pb = btop;                 // staging cursor: block it + NSP - LAG of this ring
     auto advance = [&]() {
-        if (pb > (pk * C::NB8)) {
+        if (pb > bbot(pk)) {
             --pb;
         } else {
             pk += P;
-            pb = bhi;
+            pb = btop;
         }
     };
     auto stage_cursor = [&](uint32_t st) {
@@ -232,7 +234,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                      lane);
     };
     for (int i = 0; i < NSP - LAG; ++i) {
-        if (member == 0 && pk < K0) stage_cursor((uint32_t)i);
+        if (member == 0 && pk < a.ke) stage_cursor((uint32_t)i);
         advance();
     }
 
@@ -241,14 +243,14 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     double Xr[NG][NT + 1][2], Xi[NG][NT + 1][2], TA[NG][4], TB[NG][4];
     uint32_t it = 0;
     int duty = 0;
-    for (int64_t k = grp; k < K0; k += P) {
-        const int64_t blo = k * C::NB8;
-        const uint32_t *prev = (CP && k > 0) ? a.prog + slab * K0 + (k - 1) : nullptr;
+    for (int64_t k = a.kb + grp; k < a.ke; k += P) {
+        const int64_t blo = bbot(k);
+        const uint32_t *prev = (CP && k > a.kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
         uint32_t known = 0;
         auto wait_prev = [&](int64_t b) {
             if (CP && prev) {
-                const uint32_t need = (uint32_t)(bhi - b + NBW / 8 + 1);
+                const uint32_t need = (uint32_t)(btop - b + NBW / 8 + 1);
                 while (known < need) known = prog_read(prev);
             }
         };
@@ -261,7 +263,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
         };
         auto do_block = [&](const int64_t b, double (&T0)[NG][4]) {
             if (duty == member) {
-                if (pk < K0) {
+                if (pk < a.ke) {
                     const uint32_t st = (it + NSP - LAG) & (NSP - 1);
                     if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
                     stage_cursor(st);
@@ -328,9 +330,9 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             __syncwarp();
             if (lane == 0) {
                 mbar_arrive(bar_empty + 8 * st);
-                if (CP && b < bhi) prog_publish(mine, (uint32_t)(bhi - b));
+                if (CP && b < btop) prog_publish(mine, (uint32_t)(btop - b));
             }
-            if (fastio && (b << 3) + NBW + 8 <= N) {
+            if (fastio && (b << 3) + NBW + 8 <= a.row_end) {
                 // the block lies inside the matrix: no per-access guards (bt_wy.cuh)
                 double *pr = cb + 2 * ((b << 3) + 2 * r);
 #pragma unroll
@@ -363,16 +365,20 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             ++it;
         };
 
+        // the window above tile 0 (zero beyond the matrix; a sub-range launch reads the rows handed over)
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
 #pragma unroll
-            for (int t = 1; t <= NT; ++t) Xr[g][t][0] = Xr[g][t][1] = Xi[g][t][0] = Xi[g][t][1] = 0.0;
+            for (int t = 1; t < NT; ++t)
+                wyz_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, Xr[g][t][0], Xr[g][t][1],
+                              Xi[g][t][0], Xi[g][t][1]);
+            Xr[g][NT][0] = Xr[g][NT][1] = Xi[g][NT][0] = Xi[g][NT][1] = 0.0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) TA[g][i] = TB[g][i] = 0.0;
         }
-        load_tile0(bhi, TA);
-        load_tile0(bhi - 1, TB);
-        for (int64_t b = bhi; b >= blo; b -= 2) {
+        load_tile0(btop, TA);
+        load_tile0(btop - 1, TB);
+        for (int64_t b = btop; b >= blo; b -= 2) {
             do_block(b, TA);
             if (b - 1 >= blo) do_block(b - 1, TB);
         }
@@ -384,7 +390,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                            Xi[g][t][0], Xi[g][t][1]);
         if (CP) {
             __syncwarp();
-            if (lane == 0) prog_publish(mine, (uint32_t)(bhi - blo + 1));
+            if (lane == 0) prog_publish(mine, (uint32_t)(btop - blo + 1));
         }
     }
 }
@@ -447,8 +453,15 @@ size_t wyz_scratch_bytes(int64_t N, int64_t nev)
 }
 
 template <int NBW>
+size_t wyz_tn_bytes_range(int64_t N, int64_t kb, int64_t ke)
+{
+    return (size_t)(wy_base(N, NBW, ke) - wy_base(N, NBW, kb)) * WyzCfg<NBW>::YBLK * sizeof(double);
+}
+
+// rg: sub-range launch (bt_wy.cuh WyRange; ldq and the row shift count complex elements)
+template <int NBW>
 cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                       int nsm, void *scratch, cudaStream_t st, int force_P = 0)
+                       int nsm, void *scratch, cudaStream_t st, int force_P = 0, const WyRange &rg = WyRange())
 {
     using C = WyzCfg<NBW>;
     auto kern = bt_wyz_kernel<NBW>;
@@ -458,8 +471,13 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
     }
     const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t nslab = (nev + 7) >> 3;
-    double *tn_scratch = (double *)scratch;
-    uint32_t *prog = (uint32_t *)((char *)scratch + wyz_tn_bytes<NBW>(N));
+    WyArgs a;
+    wy_range_resolve(rg, N, NBW, a.kb, a.ke, a.b_top, a.b_bot, a.row_end);
+    if (a.ke <= a.kb) return cudaSuccess;
+    if (!rg.whole()) force_P = 1;
+    const size_t tn_bytes = rg.whole() ? wyz_tn_bytes<NBW>(N) : wyz_tn_bytes_range<NBW>(N, a.kb, a.ke);
+    double *tn_scratch = (double *)scratch - wy_base(N, NBW, a.kb) * C::YBLK;
+    uint32_t *prog = (uint32_t *)((char *)scratch + tn_bytes);
     const WyPlan pl = wy_plan(true, NBW, N, nev, nsm, force_P, 8);
     const int P = pl.P;
     cudaError_t e;
@@ -467,18 +485,17 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
         e = cudaMemsetAsync(prog, 0, (size_t)nslab * K0 * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
     }
-    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)K0);
-    wyz_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn_scratch);
+    const dim3 pgrid((unsigned)((wy_bhi(N) + C::PW) / C::PW), (unsigned)(a.ke - a.kb));
+    wyz_prepass_kernel<NBW><<<pgrid, C::PW * 32, 0, st>>>(N, hh_v, hh_tau, tn_scratch, a.kb);
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     const int64_t grid = pl.grid;
-    WyArgs a;
     a.N = N;
     a.nev = nev;
     a.ldq = ldq;
     a.hh_v = hh_v;
     a.hh_tau = hh_tau;
-    a.q = q;
+    a.q = q - 2 * rg.row0;
     a.tn = tn_scratch;
     a.prog = prog;
     a.align16 = 1;

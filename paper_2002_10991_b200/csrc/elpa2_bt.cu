@@ -134,28 +134,42 @@ cudaMemPool_t scratch_pool(cudaError_t *err)
 
 template <int NBW>
 cudaError_t run_wy(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                   int align16, cudaStream_t st, int force_P = 0)
+                   int align16, cudaStream_t st, int force_P = 0, const WyRange &rg = WyRange())
 {
     cudaError_t e;
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
-    if ((e = cudaMallocFromPoolAsync(&tn, wy_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
-    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), tn, st, force_P);
+    size_t bytes = wy_scratch_bytes<NBW>(N, nev);
+    if (!rg.whole()) {
+        int64_t kb, ke, bt, bb, re;
+        wy_range_resolve(rg, N, NBW, kb, ke, bt, bb, re);
+        if (ke <= kb) return cudaSuccess;
+        bytes = wy_tn_bytes_range<NBW>(N, kb, ke) + 256;
+    }
+    if ((e = cudaMallocFromPoolAsync(&tn, bytes, pool, st)) != cudaSuccess) return e;
+    e = launch_wy<NBW>(N, nev, hh_v, hh_tau, q, ldq, align16, sm_count(), tn, st, force_P, 0, rg);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
 
 template <int NBW>
 cudaError_t run_wyz(int64_t N, int64_t nev, const double *hh_v, const double *hh_tau, double *q, int64_t ldq,
-                    cudaStream_t st, int force_P = 0)
+                    cudaStream_t st, int force_P = 0, const WyRange &rg = WyRange())
 {
     cudaError_t e;
     cudaMemPool_t pool = scratch_pool(&e);
     if (!pool) return e;
     void *tn = nullptr;
-    if ((e = cudaMallocFromPoolAsync(&tn, wyz_scratch_bytes<NBW>(N, nev), pool, st)) != cudaSuccess) return e;
-    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), tn, st, force_P);
+    size_t bytes = wyz_scratch_bytes<NBW>(N, nev);
+    if (!rg.whole()) {
+        int64_t kb, ke, bt, bb, re;
+        wy_range_resolve(rg, N, NBW, kb, ke, bt, bb, re);
+        if (ke <= kb) return cudaSuccess;
+        bytes = wyz_tn_bytes_range<NBW>(N, kb, ke) + 256;
+    }
+    if ((e = cudaMallocFromPoolAsync(&tn, bytes, pool, st)) != cudaSuccess) return e;
+    e = launch_wyz<NBW>(N, nev, hh_v, hh_tau, q, ldq, sm_count(), tn, st, force_P, rg);
     const cudaError_t e2 = cudaFreeAsync(tn, st);
     return e != cudaSuccess ? e : e2;
 }
@@ -245,6 +259,55 @@ int run_f32(int64_t N, int nbw, int64_t nev, const float *hh_v, const float *hh_
     return 0;
 }
 
+// row-block form: see include/elpa2_bt.h
+template <bool CPLX>
+int run_rows(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau, double *q_local, int64_t ldq,
+             int64_t row0, int64_t nown, int64_t nloc, int64_t kb, int64_t ke, void *stream)
+{
+    constexpr int EW = CPLX ? 2 : 1;
+    if (N < 0) return -1;
+    if (!bt_width_ok(nbw, CPLX)) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (row0 < 0 || (row0 & 7) != 0 || row0 > N) return -8;
+    if (nown < 0 || row0 + nown > N || (row0 + nown < N && (nown & 7) != 0)) return -9;
+    const int64_t need = (row0 + nown + nbw < N ? nown + nbw : N - row0);
+    if (nloc < need || row0 + nloc > N) return -10;
+    if (kb < 0 || ke < kb) return -11;
+    if (N <= 1 || nev == 0 || nown == 0 || ke == kb) return 0;
+    if (!hh_v || ((uintptr_t)hh_v & 15) != 0) return -4;
+    if (!hh_tau || ((uintptr_t)hh_tau & (8 * EW - 1)) != 0) return -5;
+    if (!q_local || ((uintptr_t)q_local & (8 * EW - 1)) != 0) return -6;
+    if (ldq < nloc) return -7;
+    WyRange rg;
+    rg.kb = kb;
+    rg.ke = ke;
+    rg.row0 = row0;
+    rg.nown = nown;
+    rg.row_end = row0 + nloc;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e;
+    if (CPLX) {
+        switch (nbw) {
+#define X(w) case w: e = run_wyz<w>(N, nev, hh_v, hh_tau, q_local, ldq, st, 1, rg); break;
+            ELPA2_CPLX_WIDTHS(X)
+#undef X
+        default: return -2;
+        }
+    } else {
+        const int align16 = (((uintptr_t)q_local & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
+        switch (nbw) {
+#define X(w) case w: e = run_wy<w>(N, nev, hh_v, hh_tau, q_local, ldq, align16, st, 1, rg); break;
+            ELPA2_REAL_WIDTHS(X)
+#undef X
+        default: return -2;
+        }
+    }
+    if (e != cudaSuccess) return (int)e;
+    g_last_launches = 2;
+    return 0;
+}
+
 // grow-only device scratch for the host-buffer entry point
 struct Scratch {
     void *p = nullptr;
@@ -317,6 +380,21 @@ int elpa2_trans_ev_tridi_to_band_host32(int is_complex, int64_t N, int nbw, int6
     if ((e = cudaMemcpyAsync(q, g_sq.p, bq, cudaMemcpyDeviceToHost, 0)) != cudaSuccess) return (int)e;
     if ((e = cudaStreamSynchronize(0)) != cudaSuccess) return (int)e;
     return 0;
+}
+
+int elpa2_trans_ev_tridi_to_band_rows_d(int64_t N, int nbw, int64_t nev, const double *hh_v, const double *hh_tau,
+                                        double *q_local, int64_t ldq, int64_t row0, int64_t nown, int64_t nloc,
+                                        int64_t kb, int64_t ke, void *stream)
+{
+    return run_rows<false>(N, nbw, nev, hh_v, hh_tau, q_local, ldq, row0, nown, nloc, kb, ke, stream);
+}
+
+int elpa2_trans_ev_tridi_to_band_rows_z(int64_t N, int nbw, int64_t nev, const void *hh_v, const void *hh_tau,
+                                        void *q_local, int64_t ldq, int64_t row0, int64_t nown, int64_t nloc,
+                                        int64_t kb, int64_t ke, void *stream)
+{
+    return run_rows<true>(N, nbw, nev, (const double *)hh_v, (const double *)hh_tau, (double *)q_local, ldq, row0, nown,
+                          nloc, kb, ke, stream);
 }
 
 int elpa2_trans_ev_tridi_to_band_host(int is_complex, int64_t N, int nbw, int64_t nev, const void *hh_v,
