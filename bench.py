@@ -470,6 +470,81 @@ def run_b2f(args, rank, world, local_rank, dist) -> None:
         dist.destroy_process_group()
 
 
+def run_rowpipe(args, rank, world, local_rank, dist) -> None:
+    """--row-pipeline R: SURVEY.md 8(f) NEXT-3.  One step = the whole back-transformation of
+    the config's N x nev block with the rows spread over R ranks (paper_2002_10991_b200/rowpipe.py).
+    world > 1: R = world real ranks, "scaling": "strong", value = model flops / max-over-ranks time.
+    world == 1: R emulated ranks on this device, one after another."""
+    import torch
+
+    from paper_2002_10991_b200 import binding, rowpipe, shard, synth_inputs as si
+
+    cplx, N, nbw, nev, seed_r, seed_x = CONFIGS[args.config]
+    R = world if world > 1 else args.row_pipeline
+    flops = model_flops(cplx, N, nev)
+    lengths = binding.hh_lengths(N, nbw)
+    hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
+    bounds = rowpipe.partition_rows(N, R, nbw)
+    mine = range(R) if world == 1 else [rank]
+    dt = torch.complex128 if cplx else torch.float64
+    gen = torch.Generator(device="cuda")
+    bufs = {}
+    for r in mine:
+        n = rowpipe.local_rows(N, nbw, bounds, r)
+        gen.manual_seed(seed_x + r)
+        back = torch.randn((nev, n, 2) if cplx else (nev, n), generator=gen, device="cuda", dtype=torch.float64)
+        bufs[r] = (torch.view_as_complex(back) if cplx else back).t()          # (n, nev) column-major, ldq = n
+    apply_fn = rowpipe.device_apply(N, nbw, hh_v, hh_tau)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        if world == 1:
+            rowpipe.run_emulated(N, nbw, bounds, [bufs[r] for r in range(R)], apply_fn)
+        else:
+            rowpipe.run(N, nbw, bounds, bufs[rank], dist, apply_fn)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    dmma_tf = binding.probe_fp64(1, 8192, 20)
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clocks:
+        barrier()
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        barrier()
+    ms = shard.max_over_ranks(e0.elapsed_time(e1), dist, "cuda") / args.steps
+    if rank == 0:
+        nops = sum(1 for r in range(R) for o in rowpipe.schedule(N, nbw, bounds, r) if o.kind == "apply")
+        nmsg = sum(1 for r in range(R) for o in rowpipe.schedule(N, nbw, bounds, r) if o.kind == "send")
+        achieved = flops / (ms * 1e-3) / 1e12
+        print(json.dumps({
+            "metric": METRIC, "value": flops / (ms * 1e-3) / 1e9, "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": workload_name(args.config) + f" [row pipeline, R = {R}"
+                                   + (" emulated on one device" if world == 1 else " ranks") + "]",
+                       "N": N, "nbw": nbw, "nev": nev, "row_bounds": bounds, "row_block_calls_per_step": nops,
+                       "halo_messages_per_step": nmsg, "halo_message_bytes": nbw * nev * (16 if cplx else 8),
+                       "parallelism": f"rows over {R} ranks, nbw-row halos" + (" over NCCL" if world > 1 else " (device copies)"),
+                       "source_sha": source_sha()},
+            "roofline": {"bound": "tensor", "achieved": achieved, "peak": dmma_tf * max(world, 1), "unit": "TFLOP/s",
+                         "frac": achieved / (dmma_tf * max(world, 1)),
+                         "peak_source": "FP64 DMMA probe of rank 0 x ranks", "kernel": "bt_wy(z)_kernel, sub-range launches",
+                         "kernel_ms": ms, "algorithmic_flops_per_launch": flops, "traffic": None},
+            "clocks": clocks.summary(), "e2e": None, "gpu_launches": 2 * nops * args.steps, "cpu_baseline": None,
+        }), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -488,6 +563,11 @@ def main() -> None:
                          "band -> full back-transformation on the same config's N, nbw, nev")
     ap.add_argument("--nev-frac", type=float, default=None,
                     help="partial spectrum (PAPER.md:218): replace nev by round(frac * N)")
+    ap.add_argument("--row-pipeline", type=int, default=0, metavar="R",
+                    help="SURVEY 8(f) NEXT-3: time the row-pipelined form instead (strong scaling over rows).  Under "
+                         "torchrun every rank owns a block of rows of ALL nev columns and hands nbw-row halos over NCCL; "
+                         "on one GPU, R ranks are emulated one after another on the same device (the sum of all ranks' "
+                         "work: measures the cost of the row-block form, not a speed-up)")
     ap.add_argument("--dtype", default="f64", choices=["f64", "f32"],
                     help="f32: SURVEY 8(f) NEXT-4, the FP32 calls elpa2_trans_ev_tridi_to_band_{s,c} on the config's shape "
                          "(step 6d only; real nbw <= 128, complex nbw <= 64)")
@@ -540,6 +620,9 @@ def main() -> None:
         return
     if args.step == "6e":
         run_b2f(args, rank, world, local_rank, dist)
+        return
+    if args.row_pipeline > 0:
+        run_rowpipe(args, rank, world, local_rank, dist)
         return
 
     # ---- inputs, generated on the device (each rank: its own nev columns, same reflectors) ----
