@@ -563,6 +563,10 @@ def main() -> None:
                          "band -> full back-transformation on the same config's N, nbw, nev")
     ap.add_argument("--nev-frac", type=float, default=None,
                     help="partial spectrum (PAPER.md:218): replace nev by round(frac * N)")
+    ap.add_argument("--reflectors", default="chase", choices=["chase", "synthetic"],
+                    help="step 6d: 'chase' (default) = the reflectors BASELINE.json specifies, produced on the device by "
+                         "elpa2_bulge_chase_{d,z} from the config's seeded band matrix (bit-identical to the oracle's chase: "
+                         "tests/test_gpu_configs.py), outside the timed region; 'synthetic' = the seeded unitary stream")
     ap.add_argument("--row-pipeline", type=int, default=0, metavar="R",
                     help="SURVEY 8(f) NEXT-3: time the row-pipelined form instead (strong scaling over rows).  Under "
                          "torchrun every rank owns a block of rows of ALL nev columns and hands nbw-row halos over NCCL; "
@@ -629,7 +633,21 @@ def main() -> None:
     lengths = binding.hh_lengths(N, nbw)
     G = int(lengths.shape[0])
     assert G == binding.hh_count(N, nbw)
-    hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
+    chase_ms = None
+    if args.reflectors == "chase" and nbw in (32, 64, 128):
+        ab = torch.from_numpy(np.ascontiguousarray(si.band_matrix(N, nbw, seed_r, cplx).T)).cuda()
+        c0, c1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        c0.record()
+        hh_v, hh_tau, _d, _e = binding.bulge_chase(N, nbw, ab)
+        c1.record()
+        torch.cuda.synchronize()
+        chase_ms = c0.elapsed_time(c1)
+        del ab, _d, _e
+        reflector_text = ("GPU bulge chase (elpa2_bulge_chase) of the config's seeded band matrix, seed %d: "
+                          "BASELINE.json's reflectors, untimed (%.0f ms)" % (seed_r, chase_ms))
+    else:
+        hh_v, hh_tau = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cuda")
+        reflector_text = "synthetic unitary stream, device-generated (DESIGN.md input recipe)"
     q = si.gaussian_block(N, nev, seed_x + 7919 * rank, cplx, "cuda")
     single = args.dtype == "f32"
     if single:
@@ -730,7 +748,7 @@ def main() -> None:
             "scaling": "weak", "vs_baseline": None, "dtype": args.dtype, "data": "synthetic",
             "config": {"workload": workload_name(args.config) + (" [FP32 arithmetic]" if single else ""), "N": N, "nbw": nbw, "nev_per_gpu": nev,
                        "reflector_slots": G,
-                       "reflectors": "synthetic unitary stream, device-generated (DESIGN.md input recipe)",
+                       "reflectors": reflector_text,
                        "l2": ("inputs larger than L2 (%.2f GiB of q + reflectors per step)"
                               % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
                              else "inputs smaller than L2; config is latency-bound (DESIGN.md)",

@@ -224,30 +224,31 @@ __device__ __forceinline__ uint32_t prog_read(const uint32_t *p)
 
 // ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column ------------------------------------------
 template <bool CG = false>
-__device__ __forceinline__ void wy_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &x0,
-                                         double &x1)
+__device__ __forceinline__ void wy_load2(const WyArgs &a, const int64_t nrow, const double *colp, bool colok, int64_t row,
+                                         double &x0, double &x1)
 {
     x0 = 0.0;
     x1 = 0.0;
-    if (!colok || row >= a.row_end) return;
-    if (a.align16 && row + 1 < a.row_end) {
+    if (!colok || row >= nrow) return;
+    if (a.align16 && row + 1 < nrow) {
         const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + row))
                              : *reinterpret_cast<const double2 *>(colp + row);
         x0 = v.x;
         x1 = v.y;
     } else {
         x0 = CG ? __ldcg(colp + row) : colp[row];
-        if (row + 1 < a.row_end) x1 = CG ? __ldcg(colp + row + 1) : colp[row + 1];
+        if (row + 1 < nrow) x1 = CG ? __ldcg(colp + row + 1) : colp[row + 1];
     }
 }
-__device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double x0, double x1)
+__device__ __forceinline__ void wy_store2(const WyArgs &a, const int64_t nrow, double *colp, bool colok, int64_t row, double x0,
+                                          double x1)
 {
-    if (!colok || row >= a.row_end) return;
-    if (a.align16 && row + 1 < a.row_end) {
+    if (!colok || row >= nrow) return;
+    if (a.align16 && row + 1 < nrow) {
         *reinterpret_cast<double2 *>(colp + row) = make_double2(x0, x1);
     } else {
         colp[row] = x0;
-        if (row + 1 < a.row_end) colp[row + 1] = x1;
+        if (row + 1 < nrow) colp[row + 1] = x1;
     }
 }
 
@@ -255,7 +256,7 @@ __device__ __forceinline__ void wy_store2(const WyArgs &a, double *colp, bool co
 // CP = false: the 8 warps of a CTA share one ring and walk every chain (grp = 0, member = warp).
 // CP = true: a.P warps share NG slabs; warp (grp, member) walks chains grp, grp+P, .. of the slabs
 // starting at `slab`; the warps with the same grp share ring grp (NS/P stages) and are its `nmem` members.
-template <class C, int NG, bool CP>
+template <class C, int NG, bool CP, bool RG>
 __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem, const int lane, const int grp,
                                            const int member, const int nmem, const int64_t col0, const int64_t slab)
 {
@@ -271,7 +272,10 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t bhi = wy_bhi(N);                      // numbering of the blocks (scratch ids) is global
-    const int64_t btop = a.b_top;                       // first block of every chain in this launch (bhi: whole matrix)
+    // RG = false (the whole matrix) keeps every bound a compile-time function of N: the code of the full launch
+    const int64_t btop = RG ? a.b_top : bhi;
+    const int64_t nrow = RG ? a.row_end : N;            // rows >= nrow are not in memory
+    const int64_t kb = RG ? a.kb : 0, ke = RG ? a.ke : K0;
     const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1
@@ -283,8 +287,8 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     const bool fastio = a.align16 && (col0 + 8 * NG <= a.nev);
 
     // staging cursor: block it + NSP - LAG of this ring's sequence
-    auto bbot = [&](int64_t k) { return k * C::NB8 > a.b_bot ? k * C::NB8 : a.b_bot; };   // last block of chain k here
-    int64_t pk = a.kb + grp, pb = btop;
+    auto bbot = [&](int64_t k) { return (RG && k * C::NB8 < a.b_bot) ? a.b_bot : k * C::NB8; };   // last block of chain k here
+    int64_t pk = kb + grp, pb = btop;
     auto advance = [&]() {
         if (pb > bbot(pk)) {
             --pb;
@@ -299,7 +303,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     };
     // prologue: blocks 0 .. NSP-LAG-1 go into fresh stages
     for (int i = 0; i < NSP - LAG; ++i) {
-        if (member == 0 && pk < a.ke) stage_cursor((uint32_t)i);
+        if (member == 0 && pk < ke) stage_cursor((uint32_t)i);
         advance();
     }
 
@@ -313,10 +317,10 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
     double X[NG][NT + 1][2], TA[NG][2], TB[NG][2];
     uint32_t it = 0;                   // blocks consumed from this ring
     int duty = 0;
-    for (int64_t k = a.kb + grp; k < a.ke; k += P) {
+    for (int64_t k = kb + grp; k < ke; k += P) {
         const int64_t blo = bbot(k);
         // chain-parallel hand-over: chain k-1 of this slab is walked by another warp of the CTA
-        const uint32_t *prev = (CP && k > a.kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
+        const uint32_t *prev = (CP && k > kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
         uint32_t known = 0;
         auto wait_prev = [&](int64_t b) {          // before loading tile 0 of block b
@@ -330,14 +334,14 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             wait_prev(b);
 #pragma unroll
             for (int g = 0; g < NG; ++g)
-                wy_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1]);
+                wy_load2<CP>(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1]);
         };
         // one block: T0 = its tile 0 on entry, tile 0 of block b - (PF2 ? 2 : 1) on exit
         auto do_block = [&](const int64_t b, double (&T0)[NG][2]) {
             // --- staging duty: block it+NSP-LAG goes into the stage that block it-LAG used; the warp
             //     on duty only waits if some member is still LAG blocks behind it
             if (duty == member) {
-                if (pk < a.ke) {
+                if (pk < ke) {
                     const uint32_t st = (it + NSP - LAG) & (NSP - 1);
                     if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
                     stage_cursor(st);
@@ -401,7 +405,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             }
             // --- tile NT-1 retires (rows 8b + nbw ..), the buffer of tile 0 is refilled
             const int64_t bn = b - (PF2 ? 2 : 1);
-            if (fastio && (b << 3) + NBW + 8 <= a.row_end) {
+            if (fastio && (b << 3) + NBW + 8 <= nrow) {
                 double *pr = cb + (b << 3) + 2 * r;
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
@@ -420,7 +424,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
             } else {
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
-                    wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
+                    wy_store2(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, X[g][NT][0], X[g][NT][1]);
                 load_tile0(bn, T0);
             }
             ++it;
@@ -432,8 +436,12 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
 #pragma unroll
-            for (int t = 1; t < NT; ++t)
-                wy_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, X[g][t][0], X[g][t][1]);
+            for (int t = 1; t < NT; ++t) {
+                if (RG)
+                    wy_load2<CP>(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, X[g][t][0], X[g][t][1]);
+                else
+                    X[g][t][0] = X[g][t][1] = 0.0;
+            }
             X[g][NT][0] = X[g][NT][1] = 0.0;
             TA[g][0] = TA[g][1] = TB[g][0] = TB[g][1] = 0.0;
         }
@@ -452,7 +460,7 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
         for (int g = 0; g < NG; ++g)
 #pragma unroll
             for (int t = 1; t < NT; ++t)
-                wy_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
+                wy_store2(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, X[g][t][0], X[g][t][1]);
         if (CP) {
             __syncwarp();
             if (lane == 0) prog_publish(mine, (uint32_t)(btop - blo + 1));
@@ -465,7 +473,8 @@ __device__ __forceinline__ void wy_consume(const WyArgs &a, unsigned char *smem,
 //  P = 1: at most NW*NGMAX slabs per CTA; warp w takes n/NW of them, +1 for the first n%NW warps
 //         (warps w and w+4 share a sub-partition, so the extras land on different sub-partitions first).
 //  P > 1 (few slabs): at most NW/P slabs per CTA; warp w works on slab w/P, chains (w%P) + m P.
-template <int NBW, int NWARPS>
+// RG: the sub-range build (rows call of SURVEY 8(f) NEXT-3; P = 1 only).  RG = false is the whole-matrix launch.
+template <int NBW, int NWARPS, bool RG = false>
 __global__ void __launch_bounds__(NWARPS * 32, 1) bt_wy_kernel(const WyArgs a)
 {
     using C = WyCfg<NBW, NWARPS>;
@@ -495,7 +504,7 @@ __global__ void __launch_bounds__(NWARPS * 32, 1) bt_wy_kernel(const WyArgs a)
     }
     __syncthreads();
 
-    if (a.P > 1) {
+    if (!RG && a.P > 1) {
         // chain-parallel: `member` = the a.P warps that share slabs; member slots NW / P
         const int grp = warp % a.P, member = warp / a.P, nm = NW / a.P;
         const int base = nmine / nm, extra = nmine % nm;
@@ -503,13 +512,13 @@ __global__ void __launch_bounds__(NWARPS * 32, 1) bt_wy_kernel(const WyArgs a)
         const int64_t wslab0 = slab0 + (int64_t)member * base + (member < extra ? member : extra);
         if (ng == 0) return;
         if (NGMAX >= 4 && ng == 4)
-            wy_consume<C, (NGMAX >= 4 ? 4 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+            wy_consume<C, (NGMAX >= 4 ? 4 : 1), true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         else if (NGMAX >= 3 && ng == 3)
-            wy_consume<C, (NGMAX >= 3 ? 3 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+            wy_consume<C, (NGMAX >= 3 ? 3 : 1), true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         else if (NGMAX >= 2 && ng == 2)
-            wy_consume<C, (NGMAX >= 2 ? 2 : 1), true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+            wy_consume<C, (NGMAX >= 2 ? 2 : 1), true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         else
-            wy_consume<C, 1, true>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+            wy_consume<C, 1, true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         return;
     }
     if (NWARPS > 8) return;                            // the 16-warp build is chain-parallel only
@@ -519,13 +528,13 @@ __global__ void __launch_bounds__(NWARPS * 32, 1) bt_wy_kernel(const WyArgs a)
     if (ng == 0) return;
     const int64_t col0 = wslab0 << 3;
     if (NGMAX >= 4 && ng == 4)
-        wy_consume<C, (NGMAX >= 4 ? 4 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wy_consume<C, (NGMAX >= 4 ? 4 : 1), false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (NGMAX >= 3 && ng == 3)
-        wy_consume<C, (NGMAX >= 3 ? 3 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wy_consume<C, (NGMAX >= 3 ? 3 : 1), false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (NGMAX >= 2 && ng == 2)
-        wy_consume<C, (NGMAX >= 2 ? 2 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wy_consume<C, (NGMAX >= 2 ? 2 : 1), false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else if (NWARPS <= 8)
-        wy_consume<C, 1, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wy_consume<C, 1, false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
 }
 
 // ---- host side -----------------------------------------------------------------------------------------
@@ -581,11 +590,11 @@ size_t wy_scratch_bytes(int64_t N, int64_t nev)
     return wy_tn_bytes<NBW>(N) + ((prog + 255) & ~(size_t)255);
 }
 
-template <int NBW, int NWARPS>
+template <int NBW, int NWARPS, bool RG = false>
 cudaError_t launch_wy_main(const WyArgs &a, const WyPlan &pl, cudaStream_t st)
 {
     using C = WyCfg<NBW, NWARPS>;
-    auto kern = bt_wy_kernel<NBW, NWARPS>;
+    auto kern = bt_wy_kernel<NBW, NWARPS, RG>;
     {
         cudaError_t e = set_max_smem((const void *)kern, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;
@@ -665,6 +674,7 @@ cudaError_t launch_wy(int64_t N, int64_t nev, const double *hh_v, const double *
     a.prog = prog;
     a.align16 = align16;
     a.P = P;
+    if (!rg.whole()) return launch_wy_main<NBW, 8, true>(a, pl, st);
     if (pl.nwarps == 16) return launch_wy_main<(NBW <= 64 ? NBW : 64), 16>(a, pl, st);
     return launch_wy_main<NBW, 8>(a, pl, st);
 }

@@ -169,33 +169,33 @@ __device__ __forceinline__ void wyz_stage(const WyArgs &a, double *stage, uint32
 
 // ---- tile I/O: rows row0 + 2r + {0,1} of this lane's column (interleaved in memory, planar in regs) ----
 template <bool CG = false>
-__device__ __forceinline__ void wyz_load2(const WyArgs &a, const double *colp, bool colok, int64_t row, double &xr0,
+__device__ __forceinline__ void wyz_load2(const WyArgs &a, const int64_t nrow, const double *colp, bool colok, int64_t row, double &xr0,
                                           double &xr1, double &xi0, double &xi1)
 {
     xr0 = xr1 = xi0 = xi1 = 0.0;
-    if (!colok || row >= a.row_end) return;
+    if (!colok || row >= nrow) return;
     const double2 v = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row))
                          : *reinterpret_cast<const double2 *>(colp + 2 * row);
     xr0 = v.x;
     xi0 = v.y;
-    if (row + 1 < a.row_end) {
+    if (row + 1 < nrow) {
         const double2 w = CG ? __ldcg(reinterpret_cast<const double2 *>(colp + 2 * row + 2))
                              : *reinterpret_cast<const double2 *>(colp + 2 * row + 2);
         xr1 = w.x;
         xi1 = w.y;
     }
 }
-__device__ __forceinline__ void wyz_store2(const WyArgs &a, double *colp, bool colok, int64_t row, double xr0,
+__device__ __forceinline__ void wyz_store2(const WyArgs &a, const int64_t nrow, double *colp, bool colok, int64_t row, double xr0,
                                            double xr1, double xi0, double xi1)
 {
-    if (!colok || row >= a.row_end) return;
+    if (!colok || row >= nrow) return;
     *reinterpret_cast<double2 *>(colp + 2 * row) = make_double2(xr0, xi0);
-    if (row + 1 < a.row_end) *reinterpret_cast<double2 *>(colp + 2 * row + 2) = make_double2(xr1, xi1);
+    if (row + 1 < nrow) *reinterpret_cast<double2 *>(colp + 2 * row + 2) = make_double2(xr1, xi1);
 }
 
 // ---- a warp with NG slabs of 8 columns -------------------------------------------------------------------
 // Same structure as wy_consume (bt_wy.cuh): CP = chain-parallel mode (a.P warps per slab, NG = 1).
-template <class C, int NG, bool CP>
+template <class C, int NG, bool CP, bool RG>
 __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem, const int lane, const int grp,
                                             const int member, const int nmem, const int64_t col0, const int64_t slab)
 {
@@ -210,7 +210,10 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     const int64_t N = a.N;
     const int64_t K0 = wy_nchains(N, C::NBW);
     const int64_t bhi = wy_bhi(N);                      // numbering of the blocks (scratch ids) is global
-    const int64_t btop = a.b_top;                       // first block of every chain in this launch (bt_wy.cuh)
+    // RG = false (the whole matrix) keeps every bound a compile-time function of N: the code of the full launch
+    const int64_t btop = RG ? a.b_top : bhi;
+    const int64_t nrow = RG ? a.row_end : N;            // rows >= nrow are not in memory
+    const int64_t kb = RG ? a.kb : 0, ke = RG ? a.ke : K0;                       // first block of every chain in this launch (bt_wy.cuh)
     const int64_t FN1 = hh_F(N - 1, C::NBW);
 
     // this lane's columns: col0 + 8g + gq, g = 0 .. NG-1 (ldq counts complex elements)
@@ -219,8 +222,8 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     const int64_t ncolrem = a.nev - col0 - gq;          // column g is valid iff 8g < ncolrem
     const bool fastio = col0 + 8 * NG <= a.nev;         // warp-uniform: every column of the warp exists
 
-    auto bbot = [&](int64_t k) { return k * C::NB8 > a.b_bot ? k * C::NB8 : a.b_bot; };   // last block of chain k here
-    int64_t pk = a.kb + grp, pb = btop;                 // staging cursor: block it + NSP - LAG of this ring
+    auto bbot = [&](int64_t k) { return (RG && k * C::NB8 < a.b_bot) ? a.b_bot : k * C::NB8; };   // last block of chain k here
+    int64_t pk = kb + grp, pb = btop;                 // staging cursor: block it + NSP - LAG of this ring
     auto advance = [&]() {
         if (pb > bbot(pk)) {
             --pb;
@@ -234,7 +237,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                      lane);
     };
     for (int i = 0; i < NSP - LAG; ++i) {
-        if (member == 0 && pk < a.ke) stage_cursor((uint32_t)i);
+        if (member == 0 && pk < ke) stage_cursor((uint32_t)i);
         advance();
     }
 
@@ -243,9 +246,9 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
     double Xr[NG][NT + 1][2], Xi[NG][NT + 1][2], TA[NG][4], TB[NG][4];
     uint32_t it = 0;
     int duty = 0;
-    for (int64_t k = a.kb + grp; k < a.ke; k += P) {
+    for (int64_t k = kb + grp; k < ke; k += P) {
         const int64_t blo = bbot(k);
-        const uint32_t *prev = (CP && k > a.kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
+        const uint32_t *prev = (CP && k > kb) ? a.prog + slab * K0 + (k - 1) : nullptr;
         uint32_t *mine = CP ? a.prog + slab * K0 + k : nullptr;
         uint32_t known = 0;
         auto wait_prev = [&](int64_t b) {
@@ -259,11 +262,11 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             wait_prev(b);
 #pragma unroll
             for (int g = 0; g < NG; ++g)
-                wyz_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1], T0[g][2], T0[g][3]);
+                wyz_load2<CP>(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + 2 * r, T0[g][0], T0[g][1], T0[g][2], T0[g][3]);
         };
         auto do_block = [&](const int64_t b, double (&T0)[NG][4]) {
             if (duty == member) {
-                if (pk < a.ke) {
+                if (pk < ke) {
                     const uint32_t st = (it + NSP - LAG) & (NSP - 1);
                     if (it >= (uint32_t)LAG) mbar_wait(bar_empty + 8 * st, ((it - LAG) >> lgs) & 1);
                     stage_cursor(st);
@@ -332,7 +335,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
                 mbar_arrive(bar_empty + 8 * st);
                 if (CP && b < btop) prog_publish(mine, (uint32_t)(btop - b));
             }
-            if (fastio && (b << 3) + NBW + 8 <= a.row_end) {
+            if (fastio && (b << 3) + NBW + 8 <= nrow) {
                 // the block lies inside the matrix: no per-access guards (bt_wy.cuh)
                 double *pr = cb + 2 * ((b << 3) + 2 * r);
 #pragma unroll
@@ -358,7 +361,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             } else {
 #pragma unroll
                 for (int g = 0; g < NG; ++g)
-                    wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
+                    wyz_store2(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (b << 3) + NBW + 2 * r, Xr[g][NT][0], Xr[g][NT][1],
                                Xi[g][NT][0], Xi[g][NT][1]);
                 load_tile0(b - 2, T0);
             }
@@ -369,9 +372,13 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
 #pragma unroll
         for (int g = 0; g < NG; ++g) {
 #pragma unroll
-            for (int t = 1; t < NT; ++t)
-                wyz_load2<CP>(a, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, Xr[g][t][0], Xr[g][t][1],
-                              Xi[g][t][0], Xi[g][t][1]);
+            for (int t = 1; t < NT; ++t) {
+                if (RG)
+                    wyz_load2<CP>(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (btop << 3) + 8 * t + 2 * r, Xr[g][t][0], Xr[g][t][1],
+                                  Xi[g][t][0], Xi[g][t][1]);
+                else
+                    Xr[g][t][0] = Xr[g][t][1] = Xi[g][t][0] = Xi[g][t][1] = 0.0;
+            }
             Xr[g][NT][0] = Xr[g][NT][1] = Xi[g][NT][0] = Xi[g][NT][1] = 0.0;
 #pragma unroll
             for (int i = 0; i < 4; ++i) TA[g][i] = TB[g][i] = 0.0;
@@ -386,7 +393,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
         for (int g = 0; g < NG; ++g)
 #pragma unroll
             for (int t = 1; t < NT; ++t)
-                wyz_store2(a, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, Xr[g][t][0], Xr[g][t][1],
+                wyz_store2(a, nrow, cb + g * ldq8, 8 * g < ncolrem, (blo << 3) + 8 * (t - 1) + 2 * r, Xr[g][t][0], Xr[g][t][1],
                            Xi[g][t][0], Xi[g][t][1]);
         if (CP) {
             __syncwarp();
@@ -396,7 +403,7 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
 }
 
 // ---- the kernel --------------------------------------------------------------------------------------------
-template <int NBW>
+template <int NBW, bool RG = false>
 __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
 {
     using C = WyzCfg<NBW>;
@@ -423,10 +430,10 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     }
     __syncthreads();
 
-    if (a.P > 1) {
+    if (!RG && a.P > 1) {
         const int grp = warp % a.P, member = warp / a.P;
         if (member >= nmine) return;
-        wyz_consume<C, 1, true>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
+        wyz_consume<C, 1, true, false>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
         return;
     }
     const int base = nmine / NW, extra = nmine % NW;
@@ -435,9 +442,9 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     if (ng == 0) return;
     const int64_t col0 = wslab0 << 3;
     if (NGMAX >= 2 && ng == 2)
-        wyz_consume<C, (NGMAX >= 2 ? 2 : 1), false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wyz_consume<C, (NGMAX >= 2 ? 2 : 1), false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
     else
-        wyz_consume<C, 1, false>(a, smem, lane, 0, warp, nact, col0, wslab0);
+        wyz_consume<C, 1, false, RG>(a, smem, lane, 0, warp, nact, col0, wslab0);
 }
 
 template <int NBW>
@@ -464,7 +471,7 @@ cudaError_t launch_wyz(int64_t N, int64_t nev, const double *hh_v, const double 
                        int nsm, void *scratch, cudaStream_t st, int force_P = 0, const WyRange &rg = WyRange())
 {
     using C = WyzCfg<NBW>;
-    auto kern = bt_wyz_kernel<NBW>;
+    auto kern = rg.whole() ? bt_wyz_kernel<NBW, false> : bt_wyz_kernel<NBW, true>;
     {
         cudaError_t e = set_max_smem((const void *)kern, C::SMEM_BYTES);
         if (e != cudaSuccess) return e;

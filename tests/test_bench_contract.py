@@ -45,3 +45,22 @@ def test_bench_reference_arm_runs_on_cpu():
     d = _run("--impl", "reference", "--shape", "d,300,32,64", "--steps", "1", "--warmup", "0")
     assert d["impl"] == "reference" and d["value"] > 0 and d["gpu_launches"] == 0
     assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["cpu_baseline"]["kind"] == "oracle"
+
+
+@pytest.mark.gpu
+def test_bench_default_line_times_chase_reflectors():
+    d = _run("--shape", "d,700,64,600", "--e2e-steps", "0", "--no-cpu-baseline")
+    assert d["config"]["reflectors"].startswith("GPU bulge chase")
+    d = _run("--shape", "d,700,64,600", "--e2e-steps", "0", "--no-cpu-baseline", "--reflectors", "synthetic")
+    assert d["config"]["reflectors"].startswith("synthetic")
+
+
+@pytest.mark.gpu
+def test_bench_other_lines():
+    d = _run("--dtype", "f32", "--shape", "z,500,64,300", "--e2e-steps", "1")
+    assert d["dtype"] == "f32" and d["roofline"]["bound"] == "alu" and d["gpu_launches"] >= 2 and "FP32" in d["metric"]
+    assert d["checks"]["max_rel_column_norm_drift_after_all_steps"] < 1e-4
+    d = _run("--step", "6e", "--shape", "z,600,64,300", "--e2e-steps", "1")
+    assert d["metric"].startswith("band->full") and d["roofline"]["kernel"].startswith("bt_b2fz_kernel")
+    d = _run("--row-pipeline", "3", "--shape", "d,900,64,200")
+    assert d["scaling"] == "strong" and d["config"]["halo_messages_per_step"] > 0 and d["value"] > 0
