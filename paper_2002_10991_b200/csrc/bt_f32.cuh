@@ -34,7 +34,11 @@ struct F32Cfg {
     static constexpr int NS = 8, LGNS = 3, LAG = 4;   // ring
     static constexpr int V_FLOATS = 8 * NBW * EW;     // V[i][r] (interleaved for complex)
     static constexpr int STAGE_FLOATS = V_FLOATS + 16;// + tau[8] (re, im)
-    static constexpr int OFF_BAR = NS * STAGE_FLOATS * 4;
+    // per-warp ring of incoming 8-row tiles of q: [16-byte piece][lane][4 floats], filled by the lane's own cp.async
+    static constexpr int NSQ = 4, DQ = 3;             // stages, tiles fetched ahead
+    static constexpr int QTILE = 8 * 32 * EW;         // floats per tile
+    static constexpr int OFF_Q = NS * STAGE_FLOATS * 4;
+    static constexpr int OFF_BAR = OFF_Q + NW * NSQ * QTILE * 4;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
     static_assert(NBW % 32 == 0, "nbw");
 };
@@ -77,40 +81,45 @@ __device__ __forceinline__ void f32_stage(const F32Args &a, float *stage, uint32
     cp_async_mbar_arrive_noinc_wy(bar_full);
 }
 
-// ---- 8 rows of this lane's column: rows row0 .. row0+7 (row0 a multiple of 8) ------------------------------
+// ---- 8 rows of this lane's column (rows row0 .. row0+7, row0 a multiple of 8) on their way in ---------------------
+// f32_fetch8: the lane's own cp.async copies into its slots of the warp's tile (zero fill beyond N and for
+// absent columns / blocks); f32_take8: the same lane reads them back once its copy group has completed.
 template <bool CPLX>
-__device__ __forceinline__ void f32_load8(const F32Args &a, const float *colp, bool colok, int64_t row0, float (&r)[8],
-                                          float (&im)[8])
+__device__ __forceinline__ void f32_fetch8(const F32Args &a, const float *colp, bool ok, int64_t row0, float *tile, int lane)
 {
+    constexpr int EW = CPLX ? 2 : 1, NP = 2 * EW;     // 16-byte pieces: 4 / EW rows each
+    const int64_t left = ok ? a.N - row0 : 0;         // rows present from row0 on
+    if (a.align16) {
 #pragma unroll
-    for (int e = 0; e < 8; ++e) r[e] = im[e] = 0.0f;
-    if (!colok || row0 >= a.N || row0 < 0) return;
-    if (a.align16 && row0 + 8 <= a.N) {
-        if (CPLX) {
-#pragma unroll
-            for (int h = 0; h < 4; ++h) {
-                const float4 v = *reinterpret_cast<const float4 *>(colp + 2 * row0 + 4 * h);
-                r[2 * h] = v.x, im[2 * h] = v.y, r[2 * h + 1] = v.z, im[2 * h + 1] = v.w;
-            }
-        } else {
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const float4 v = *reinterpret_cast<const float4 *>(colp + row0 + 4 * h);
-                r[4 * h] = v.x, r[4 * h + 1] = v.y, r[4 * h + 2] = v.z, r[4 * h + 3] = v.w;
-            }
+        for (int h = 0; h < NP; ++h) {
+            int64_t nr = left - h * (4 / EW);
+            nr = nr < 0 ? 0 : (nr > 4 / EW ? 4 / EW : nr);
+            cp_async16(smem_u32(tile + (h * 32 + lane) * 4), nr ? colp + (row0 * EW + 4 * h) : a.q, (uint32_t)(nr * 4 * EW));
         }
-        return;
+    } else {
+#pragma unroll
+        for (int e = 0; e < 8 * EW; ++e) {
+            const bool in = (e / EW) < left;
+            cp_async4(smem_u32(tile + ((e >> 2) * 32 + lane) * 4 + (e & 3)), in ? colp + (row0 * EW + e) : a.q, in ? 4u : 0u);
+        }
     }
+}
+template <bool CPLX>
+__device__ __forceinline__ void f32_take8(const float *tile, int lane, float *r, float *im)
+{
+    if (CPLX) {
 #pragma unroll
-    for (int e = 0; e < 8; ++e)
-        if (row0 + e < a.N) {
-            if (CPLX) {
-                r[e] = colp[2 * (row0 + e)];
-                im[e] = colp[2 * (row0 + e) + 1];
-            } else {
-                r[e] = colp[row0 + e];
-            }
+        for (int h = 0; h < 4; ++h) {
+            const float4 v = *reinterpret_cast<const float4 *>(tile + (h * 32 + lane) * 4);
+            r[2 * h] = v.x, im[2 * h] = v.y, r[2 * h + 1] = v.z, im[2 * h + 1] = v.w;
         }
+    } else {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const float4 v = *reinterpret_cast<const float4 *>(tile + (h * 32 + lane) * 4);
+            r[4 * h] = v.x, r[4 * h + 1] = v.y, r[4 * h + 2] = v.z, r[4 * h + 3] = v.w;
+        }
+    }
 }
 
 template <bool CPLX>
@@ -142,19 +151,41 @@ __device__ __forceinline__ void f32_store8(const F32Args &a, float *colp, bool c
         }
 }
 
-// LDS.128 the compiler may not merge with an earlier load of the same address: with nbw * EW > 64 the
-// reflector is read twice (dot product, update) instead of being kept in nbw * EW registers next to the window
-__device__ __forceinline__ float4 lds128_again(const float *p)
+// ---- reading a reflector from shared memory ----------------------------------------------------------------
+// body(j, v4) for the NL broadcast LDS.128 of a reflector, ascending (dot product) or descending (update).
+// CH = 0: plain loads; ptxas keeps the reflector in registers between the two passes and hoists loads as it
+// likes -- right for narrow windows.  CH > 0 (wide windows, where that costs spills): the loads go in
+// chunks of CH, chunk c+1 issued before the arithmetic of chunk c, and a __syncwarp() between chunks keeps
+// later loads from being hoisted above it (it orders shared-memory accesses): at most 2 CH float4 are live.
+template <int NL, int CH, bool DESC, class F>
+__device__ __forceinline__ void f32_for_v(const float *v, F &&body)
 {
-    float4 v;
-    asm volatile("ld.shared.v4.f32 {%0,%1,%2,%3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(smem_u32(p)));
-    return v;
-}
-template <bool AGAIN>
-__device__ __forceinline__ float4 f32_v4(const float *p)
-{
-    if (AGAIN) return lds128_again(p);
-    return *reinterpret_cast<const float4 *>(p);
+    if constexpr (CH == 0) {
+#pragma unroll
+        for (int t = 0; t < NL; ++t) {
+            const int j = DESC ? NL - 1 - t : t;
+            body(j, *reinterpret_cast<const float4 *>(v + 4 * j));
+        }
+    } else {
+        constexpr int NC = NL / CH;
+        static_assert(NL % CH == 0, "chunking");
+        float4 buf[2][CH];
+#pragma unroll
+        for (int t = 0; t < CH; ++t) buf[0][t] = *reinterpret_cast<const float4 *>(v + 4 * (DESC ? NL - 1 - t : t));
+#pragma unroll
+        for (int c = 0; c < NC; ++c) {
+            __syncwarp();
+            if (c + 1 < NC) {
+#pragma unroll
+                for (int t = 0; t < CH; ++t) {
+                    const int j = DESC ? NL - 1 - ((c + 1) * CH + t) : (c + 1) * CH + t;
+                    buf[(c + 1) & 1][t] = *reinterpret_cast<const float4 *>(v + 4 * j);
+                }
+            }
+#pragma unroll
+            for (int t = 0; t < CH; ++t) body(DESC ? NL - 1 - (c * CH + t) : c * CH + t, buf[c & 1][t]);
+        }
+    }
 }
 
 // ---- one reflector on the register window --------------------------------------------------------------
@@ -164,58 +195,56 @@ __device__ __forceinline__ float4 f32_v4(const float *p)
 template <int NBW, int OFF, int SHIFT>
 __device__ __forceinline__ void f32_apply_real(float *x, const float *v, const float tau)
 {
-    float acc[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-#pragma unroll
-    for (int j = 0; j < NBW / 4; ++j) {
-        const float4 v4 = *reinterpret_cast<const float4 *>(v + 4 * j);
-        acc[0] = fmaf(v4.x, x[OFF + 4 * j], acc[0]);
-        acc[1] = fmaf(v4.y, x[OFF + 4 * j + 1], acc[1]);
-        acc[2] = fmaf(v4.z, x[OFF + 4 * j + 2], acc[2]);
-        acc[3] = fmaf(v4.w, x[OFF + 4 * j + 3], acc[3]);
-    }
-    const float ntd = -tau * ((acc[0] + acc[1]) + (acc[2] + acc[3]));
-#pragma unroll
-    for (int j = NBW / 4 - 1; j >= 0; --j) {
-        const float4 v4 = f32_v4<(NBW > 64)>(v + 4 * j);
+    constexpr int CH = (NBW > 64) ? 8 : 0;
+    // eight partial sums: with at most two warps per sub-partition the dot product must bring its own
+    // instruction-level parallelism (an FFMA result is ready after 4 cycles)
+    float acc[8] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+    f32_for_v<NBW / 4, CH, false>(v, [&](const int j, const float4 v4) {
+        const int o = 4 * (j & 1);
+        acc[o] = fmaf(v4.x, x[OFF + 4 * j], acc[o]);
+        acc[o + 1] = fmaf(v4.y, x[OFF + 4 * j + 1], acc[o + 1]);
+        acc[o + 2] = fmaf(v4.z, x[OFF + 4 * j + 2], acc[o + 2]);
+        acc[o + 3] = fmaf(v4.w, x[OFF + 4 * j + 3], acc[o + 3]);
+    });
+    const float ntd = -tau * (((acc[0] + acc[4]) + (acc[1] + acc[5])) + ((acc[2] + acc[6]) + (acc[3] + acc[7])));
+    f32_for_v<NBW / 4, CH, true>(v, [&](const int j, const float4 v4) {
         x[OFF + SHIFT + 4 * j + 3] = fmaf(ntd, v4.w, x[OFF + 4 * j + 3]);
         x[OFF + SHIFT + 4 * j + 2] = fmaf(ntd, v4.z, x[OFF + 4 * j + 2]);
         x[OFF + SHIFT + 4 * j + 1] = fmaf(ntd, v4.y, x[OFF + 4 * j + 1]);
         x[OFF + SHIFT + 4 * j] = fmaf(ntd, v4.x, x[OFF + 4 * j]);
-    }
+    });
 }
 
 // complex: v interleaved (re, im) in shared memory, x planar in registers; tau as stored, conj(v) in the dot (R2)
 template <int NBW, int OFF, int SHIFT>
 __device__ __forceinline__ void f32_apply_cplx(float *xr, float *xi, const float *v, const float taur, const float taui)
 {
-    float dr[2] = {0.0f, 0.0f}, di[2] = {0.0f, 0.0f};
-#pragma unroll
-    for (int j = 0; j < NBW / 2; ++j) {
-        const float4 v4 = *reinterpret_cast<const float4 *>(v + 4 * j);     // elements 2j, 2j+1
+    constexpr int CH = (NBW > 32) ? 4 : 0;
+    // eight independent partial sums (see f32_apply_real)
+    float dr[4] = {0.0f, 0.0f, 0.0f, 0.0f}, di[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    f32_for_v<NBW / 2, CH, false>(v, [&](const int j, const float4 v4) {      // elements 2j, 2j+1
         dr[0] = fmaf(v4.x, xr[OFF + 2 * j], dr[0]);
-        dr[0] = fmaf(v4.y, xi[OFF + 2 * j], dr[0]);
+        dr[1] = fmaf(v4.y, xi[OFF + 2 * j], dr[1]);
         di[0] = fmaf(v4.x, xi[OFF + 2 * j], di[0]);
-        di[0] = fmaf(-v4.y, xr[OFF + 2 * j], di[0]);
-        dr[1] = fmaf(v4.z, xr[OFF + 2 * j + 1], dr[1]);
-        dr[1] = fmaf(v4.w, xi[OFF + 2 * j + 1], dr[1]);
-        di[1] = fmaf(v4.z, xi[OFF + 2 * j + 1], di[1]);
-        di[1] = fmaf(-v4.w, xr[OFF + 2 * j + 1], di[1]);
-    }
-    const float dotr = dr[0] + dr[1], doti = di[0] + di[1];
+        di[1] = fmaf(-v4.y, xr[OFF + 2 * j], di[1]);
+        dr[2] = fmaf(v4.z, xr[OFF + 2 * j + 1], dr[2]);
+        dr[3] = fmaf(v4.w, xi[OFF + 2 * j + 1], dr[3]);
+        di[2] = fmaf(v4.z, xi[OFF + 2 * j + 1], di[2]);
+        di[3] = fmaf(-v4.w, xr[OFF + 2 * j + 1], di[3]);
+    });
+    const float dotr = (dr[0] + dr[1]) + (dr[2] + dr[3]), doti = (di[0] + di[1]) + (di[2] + di[3]);
     const float ntr = -(taur * dotr - taui * doti), nti = -(taur * doti + taui * dotr);   // -tau * dot
-#pragma unroll
-    for (int j = NBW / 2 - 1; j >= 0; --j) {
-        const float4 v4 = f32_v4<(2 * NBW > 64)>(v + 4 * j);
+    f32_for_v<NBW / 2, CH, true>(v, [&](const int j, const float4 v4) {
         // x += (ntr + i nti) (vr + i vi)
-        float r1 = fmaf(ntr, v4.z, xr[OFF + 2 * j + 1]);
-        float i1 = fmaf(ntr, v4.w, xi[OFF + 2 * j + 1]);
+        const float r1 = fmaf(ntr, v4.z, xr[OFF + 2 * j + 1]);
+        const float i1 = fmaf(ntr, v4.w, xi[OFF + 2 * j + 1]);
         xr[OFF + SHIFT + 2 * j + 1] = fmaf(-nti, v4.w, r1);
         xi[OFF + SHIFT + 2 * j + 1] = fmaf(nti, v4.z, i1);
-        float r0 = fmaf(ntr, v4.x, xr[OFF + 2 * j]);
-        float i0 = fmaf(ntr, v4.y, xi[OFF + 2 * j]);
+        const float r0 = fmaf(ntr, v4.x, xr[OFF + 2 * j]);
+        const float i0 = fmaf(ntr, v4.y, xi[OFF + 2 * j]);
         xr[OFF + SHIFT + 2 * j] = fmaf(-nti, v4.y, r0);
         xi[OFF + SHIFT + 2 * j] = fmaf(nti, v4.x, i0);
-    }
+    });
 }
 
 // reflectors I .. END-1 of a block
@@ -264,22 +293,33 @@ __device__ __forceinline__ void f32_consume(const F32Args &a, unsigned char *sme
         advance();
     }
     float xr[W], xi[CPLX ? W : 8];
-    float pr[8], pi[8];
+    // incoming rows travel through the warp's private shared-memory ring, DQ tiles ahead of their use: no
+    // register waits on a load in flight (with a register prefetch one block ahead a quarter of all samples
+    // sat on the first use of the loaded rows: one block of FFMAs is about one DRAM round trip)
+    float *qring = reinterpret_cast<float *>(smem + C::OFF_Q) + (size_t)member * C::NSQ * C::QTILE;
     uint32_t it = 0;
     int duty = 0;
     for (int64_t k = 0; k < K0; ++k) {
         const int64_t blo = k * C::NB8;
+        int qin = 0, qout = 0;                          // ring slots of the tile fetched next / taken next
+        auto fetch = [&](int64_t b) {                   // tile of block b (none below the chain: zeros)
+            f32_fetch8<CPLX>(a, cb, colok && b >= blo, b << 3, qring + qin * C::QTILE, lane);
+            cp_async_commit();
+            qin = (qin + 1) & (C::NSQ - 1);
+        };
+        auto take = [&]() {                             // the oldest tile in flight into window offsets 0 .. 7
+            asm volatile("cp.async.wait_group %0;" ::"n"(C::DQ - 1) : "memory");
+            f32_take8<CPLX>(qring + qout * C::QTILE, lane, xr, xi);
+            qout = (qout + 1) & (C::NSQ - 1);
+        };
 #pragma unroll
         for (int w = 0; w < W; ++w) {
             xr[w] = 0.0f;
             if (CPLX) xi[w] = 0.0f;
         }
-        f32_load8<CPLX>(a, cb, colok, bhi << 3, pr, pi);
 #pragma unroll
-        for (int e = 0; e < 8; ++e) {
-            xr[e] = pr[e];
-            if (CPLX) xi[e] = pi[e];
-        }
+        for (int i = 0; i < C::DQ; ++i) fetch(bhi - i);
+        take();
         for (int64_t b = bhi; b >= blo; --b) {
             if (duty == member && pk < K0) {
                 const uint32_t st = (it + NS - LAG) & (NS - 1);
@@ -288,8 +328,7 @@ __device__ __forceinline__ void f32_consume(const F32Args &a, unsigned char *sme
             }
             advance();
             duty = (duty + 1 == nmem) ? 0 : duty + 1;
-            // the 8 rows the window takes in after this block, one block ahead
-            f32_load8<CPLX>(a, cb, colok && b - 1 >= blo, (b - 1) << 3, pr, pi);
+            fetch(b - C::DQ);
 
             const uint32_t st = it & (NS - 1);
             mbar_wait(bar_full + 8 * st, (it >> C::LGNS) & 1);
@@ -301,13 +340,10 @@ __device__ __forceinline__ void f32_consume(const F32Args &a, unsigned char *sme
             f32_block_step<C, 7, 8>(xr, xi, V, V + C::V_FLOATS);
             __syncwarp();
             if (lane == 0) mbar_arrive(bar_empty + 8 * st);
-#pragma unroll
-            for (int e = 0; e < 8; ++e) {
-                xr[e] = pr[e];
-                if (CPLX) xi[e] = pi[e];
-            }
+            take();                                     // rows of block b-1
             ++it;
         }
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
         // chain end: offsets 8 .. W-1 hold rows 8 blo .. 8 blo + nbw - 1
 #pragma unroll
         for (int t = 0; t < C::NB8; ++t)
