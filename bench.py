@@ -556,6 +556,8 @@ def main() -> None:
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--variant", type=int, default=0, choices=[0, 1, 2, 3],
                     help="library variant for A/B runs (include/elpa2_bt.h): 0 default, 2 register window, 3 two chains per pass")
+    ap.add_argument("--chain-parallel", type=int, default=0, choices=[0, 1, 2, 4],
+                    help="testing aid: force P warps per slab in the default variant (0 = the library's plan)")
     ap.add_argument("--chase", action="store_true",
                     help="time SURVEY 8(f) NEXT-1 instead: the GPU bulge chase (real configs) that produces the reflectors")
     ap.add_argument("--step", default="6d", choices=["6d", "6e"],
@@ -658,6 +660,7 @@ def main() -> None:
         esz //= 2
     stream = torch.cuda.current_stream()
     binding.set_variant(args.variant)
+    binding.set_chain_parallel(args.chain_parallel)
 
     def step():
         binding.trans_ev_tridi_to_band(N, nbw, hh_v, hh_tau, q, stream=stream)
@@ -753,7 +756,9 @@ def main() -> None:
                               % ((G * nbw + G + 2 * N * nev) * esz / 2**30)) if (G * nbw + N * nev) * esz > 2**28
                              else "inputs smaller than L2; config is latency-bound (DESIGN.md)",
                        "parallelism": "column shards, no collective" if world > 1 else "single GPU",
-                       "variant": args.variant, "source_sha": source_sha()},
+                       "variant": args.variant, "chain_parallel": args.chain_parallel or "planned",
+                       "plan": binding.plan(cplx, N, nbw, nev, torch.cuda.get_device_properties(local_rank).multi_processor_count),
+                       "source_sha": source_sha()},
             "roofline": {"bound": "tensor" if tensor_path else "alu", "achieved": achieved, "peak": peak_tf,
                          "unit": "TFLOP/s", "frac": achieved / peak_tf,
                          "peak_source": ("FP64 %s probe measured in this run (elpa2_bt_probe_fp64 kind %d); "

@@ -371,7 +371,8 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
         }
         if (has_dot) {
             // --- W^T += q^T V_{P-1}: K = 16 rows, chunk e: k-slot r = row 4r + e; n-tile i = reflectors 8i + n.
-            //     Two n-tiles at a time: 2 NG independent accumulators in rotation
+            //     Two n-tiles at a time: 2 NG independent accumulators in rotation (splitting further -- four
+            //     chains for a one-slab warp -- was measured and changed nothing)
             const double *bp = pb + gq * S + 4 * r;
 #pragma unroll
             for (int i = 0; i < 8; i += 2) {
@@ -442,9 +443,22 @@ __device__ __forceinline__ void b2f_consume(const B2fArgs &a, unsigned char *sme
     asm volatile("cp.async.wait_group 0;" ::: "memory");
 }
 
+// slabs of the next round: rem slabs and `units` slab-passes (of 4 slabs) are left for `left` rounds
+__device__ __forceinline__ int64_t b2f_round(int64_t rem, int64_t left, int64_t &units)
+{
+    const int64_t c = (units + left - 1) / left;       // this round's share of the slab-passes
+    const int64_t later = 4 * (units - c);             // what the later rounds can take
+    int64_t nr = (rem + left - 1) / left;
+    if (nr < rem - later) nr = rem - later;
+    if (nr > 4 * c) nr = 4 * c;
+    if (nr > rem) nr = rem;
+    units -= c;
+    return nr;
+}
+
 // ---- the kernel ----------------------------------------------------------------------------------------------
 // grid: CTA c takes slabs [nslab*c/grid, nslab*(c+1)/grid) and walks them in rounds of up to NW*NGMAX = 16;
-// in a round warp w takes n/8 slabs, +1 for the first n%8 warps (warps w and w+4 share a sub-partition).
+// (equal-sized rounds); in a round warp w takes n/8 slabs, +1 for the first n%8 warps (warps w and w+4 share a sub-partition).
 // A round is one full sequence of passes; the V ring is drained and re-initialised between rounds.
 __global__ void __launch_bounds__(256, 1) bt_b2f_kernel(const B2fArgs a)
 {
@@ -457,10 +471,14 @@ __global__ void __launch_bounds__(256, 1) bt_b2f_kernel(const B2fArgs a)
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int64_t nmine = nslab * (blockIdx.x + 1) / gridDim.x - slab0;
 
-    int64_t done = 0;
-    while (done < nmine) {
-        int64_t nround = nmine - done;
-        if (nround > C::NW * C::NGMAX) nround = C::NW * C::NGMAX;
+    // Rounds: a round costs a full sequence of passes on its busiest sub-partition, i.e. ceil(slabs / 4)
+    // slab-passes.  The split keeps the sum of those at its minimum ceil(n / 4) and, within that, the rounds
+    // as even as possible: 28 slabs are 16 + 12 (4 + 3), 20 are 12 + 8, 17 are 9 + 8 -- not 16 + 4 or 16 + 1,
+    // whose last round would leave most warps idle (b2f_round, also used by the complex kernel).
+    const int64_t rounds = (nmine + C::NW * C::NGMAX - 1) / (C::NW * C::NGMAX);
+    int64_t done = 0, units = (nmine + 3) >> 2;
+    for (int64_t rd = 0; rd < rounds; ++rd) {
+        const int64_t nround = b2f_round(nmine - done, rounds - rd, units);
         const int nact = (int)(nround < C::NW ? nround : C::NW);           // warps with work = ring members
         if (threadIdx.x == 0) {
             for (int i = 0; i < C::NS; ++i) {

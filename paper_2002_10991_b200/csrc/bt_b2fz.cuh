@@ -311,10 +311,10 @@ __global__ void __launch_bounds__(256, 1) bt_b2fz_kernel(const B2fArgs a)
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int64_t nmine = nslab * (blockIdx.x + 1) / gridDim.x - slab0;
 
-    int64_t done = 0;
-    while (done < nmine) {
-        int64_t nround = nmine - done;
-        if (nround > C::NW) nround = C::NW;
+    const int64_t rounds = (nmine + C::NW - 1) / C::NW;      // rounds sized by b2f_round (bt_b2f.cuh)
+    int64_t done = 0, units = (nmine + 3) >> 2;
+    for (int64_t rd = 0; rd < rounds; ++rd) {
+        const int64_t nround = b2f_round(nmine - done, rounds - rd, units);
         const int nact = (int)nround;
         if (threadIdx.x == 0) {
             for (int i = 0; i < C::NS; ++i) {

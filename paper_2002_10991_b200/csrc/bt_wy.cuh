@@ -548,6 +548,37 @@ inline int wy_pick_P(int64_t nslab, int64_t K0, int nsm, int nw, int maxP)
     return nslab <= (int64_t)nsm * nw ? P : 1;
 }
 
+// Busiest sub-partition of a CTA that holds n slabs with P warps per slab group, in slab-passes: the 8
+// warps form 8/P groups, group m = warps mP .. mP+P-1 takes n/(8/P) slabs (+1 for the first ones) and each
+// of its warps walks 1/P of their chains; warp w issues on sub-partition w % 4, whose DMMA pipe is the
+// resource the kernel is bound by.
+inline double wy_smsp_load(int P, int64_t n)
+{
+    const int nm = 8 / P;
+    double load[4] = {0, 0, 0, 0};
+    for (int w = 0; w < 8; ++w) {
+        const int m = w / P;
+        load[w & 3] += (double)(n / nm + (m < n % nm ? 1 : 0)) / P;
+    }
+    double mx = 0;
+    for (int s = 0; s < 4; ++s) mx = load[s] > mx ? load[s] : mx;
+    return mx;
+}
+// Real kernel, one wave: the P in {1, 2, 4} that balances the sub-partitions (partial spectra, PAPER.md:218:
+// 5-16 slabs per SM).  Measured on B200 (N = 8192, nbw 64, n slabs per SM; TFLOP/s for P = 1 / 2 / 4):
+// n = 5: 15.3 / 19.8 / 25.9, 6: 18.8 / 23.7 / 26.9, 7: 22.3 / 23.6 / 27.1, 9: 21.0 / 25.7 / -, 10: 23.2 / 28.4 / -,
+// 13: 24.2 / 26.7 / -.  Up to 8 slabs P = 4 always wins (one-slab warps two to a sub-partition run the pipe
+// badly); above that P = 2 when it lowers the busiest sub-partition by more than its 3 % hand-over cost.
+inline int wy_pick_P_real(int64_t nslab, int64_t K0, int nsm, int ngmax, int maxP)
+{
+    const int64_t grid = nslab < nsm ? nslab : nsm;
+    const int64_t n = (nslab + grid - 1) / grid;
+    if (n > 8 * (int64_t)ngmax) return 1;              // more than one wave of the P = 1 launch
+    auto ok = [&](int P) { return P <= maxP && 4 * P <= K0 && n <= (int64_t)(8 / P) * ngmax; };
+    if (n <= 8) return ok(4) ? 4 : ok(2) ? 2 : 1;
+    return (ok(2) && wy_smsp_load(2, n) * 1.03 < wy_smsp_load(1, n)) ? 2 : 1;
+}
+
 // launch plan of the main kernel (pure host arithmetic; exported as elpa2_bt_plan for the CPU tests)
 struct WyPlan {
     int64_t grid;        // CTAs
@@ -568,7 +599,10 @@ inline WyPlan wy_plan(bool cplx, int nbw, int64_t N, int64_t nev, int nsm, int f
     const int ns = cplx ? (nbw <= 64 ? 8 : 4) : ((8 * 16 * (nbw + 8) * 8 <= 216 * 1024) ? 8 : 4);
     const int maxP = cplx ? 2 : (ns >= 8 ? 4 : 2);
     if (force_P > maxP) force_P = maxP;
-    pl.P = many_warps ? 4 : (force_P > 0 ? force_P : wy_pick_P(pl.nslab, K0, nsm, 8, maxP));
+    pl.P = many_warps ? 4
+           : force_P > 0 ? force_P
+           : cplx ? wy_pick_P(pl.nslab, K0, nsm, 8, maxP)
+                  : wy_pick_P_real(pl.nslab, K0, nsm, ngmax8, maxP);
     // (the complex kernel and the 16-warp build walk one slab per warp in chain-parallel mode)
     pl.per_cta = (int64_t)(pl.nwarps / pl.P) * ((many_warps || (cplx && pl.P > 1)) ? 1 : ngmax8);
     const int64_t waves = (pl.nslab + nsm * pl.per_cta - 1) / (nsm * pl.per_cta);

@@ -98,6 +98,17 @@ def test_chain_parallel_mode(nbw, cplx):
     _check(12 * nbw + 7, nbw, 148 * 8 * 3 + 5, cplx)   # 3-4 slabs per CTA: P = 2, ragged tail
 
 
+@pytest.mark.parametrize("nbw,n", [(32, 5), (64, 6), (64, 7), (64, 10), (64, 13), (128, 3), (128, 7), (96, 4)])
+def test_partial_spectrum_plans(nbw, n):
+    # 5-16 slabs per CTA: the plan shares slab groups among P = 4 / 2 warps with SEVERAL slabs per warp
+    # (the sub-partition balance of DESIGN.md 5.1); ragged last slab
+    from paper_2002_10991_b200 import binding
+
+    N, nev = 17 * nbw + 1, 148 * 8 * n - 3
+    assert binding.plan(False, N, nbw, nev, 148)["P"] in (2, 4)
+    _check(N, nbw, nev, False)
+
+
 @pytest.mark.parametrize("cplx", [False, True])
 def test_more_columns_than_one_wave(cplx):
     # more slabs than 148 CTAs x 8 warps x NGMAX: the grid becomes a multiple of the SM count > 1
