@@ -1,6 +1,6 @@
 // bt_b2fz.cuh -- band -> full back-transformation (Eq. 6e), COMPLEX FP64, on the FP64
 // tensor cores (sm_100a).  Same algorithm, ring layout and fragment chaining as bt_b2f.cuh; every complex
-// product is four real DMMAs on planar register fragments, memory stays interleaved (re, im).
+// product is THREE real DMMAs (3M form) on planar register fragments, memory stays interleaved (re, im).
 //
 //      q <- H_0 H_1 ... H_{Nv-1} q,   H_j = I - tau_j v_j v_j^H  (R2: tau as stored, v^H in the dot)
 //      blocks of 64: Q_p = I - V_p T_p V_p^H,  T upper triangular, T[i][i] = tau_i,
@@ -16,7 +16,8 @@
 //   update  B[k = r][n = gq] = V[row gq][reflector 8i+2r+e]   -> word offset 72 r + 4 gq = 8 r + 4 gq (mod 32)
 //   dot     B[k = r][n = gq] = V[row 2r+e][reflector 8i+gq]   -> word offset 36 gq + 8 r   = 4 gq + 8 r (mod 32)
 // Lane (gq, r) holds complex rows 2r, 2r+1 of column gq of an 8-row group (32 contiguous bytes).
-// A warp owns ONE slab of 8 columns for all passes: W, U and -Im U (5 x 16 doubles) live in registers.
+// A warp owns ONE slab of 8 columns for all passes: the three accumulators of W (3M form, below) and U
+// (5 x 16 doubles) live in registers.
 #pragma once
 #include "bt_b2f.cuh"
 
@@ -170,11 +171,16 @@ __device__ __forceinline__ void b2fz_consume(const B2fArgs &a, unsigned char *sm
     }
 
     // n-tile i, entry e: reflector 8i + 2r + e of this lane's column
-    double Wr[8][2], Wi[8][2], Ur[8][2], Ui[8][2], nUi[8][2];
+    // Both big products use the 3M form of a complex product (three real DMMAs instead of four; the operand
+    // sums are one DADD each on the same FP64 pipe, 2 cycles against 16):
+    //   dot:     P1 += qr Vr,  P2 += qi Vi,  P3 += (qr + qi)(Vr - Vi)   =>  Wr = P1 + P2,  Wi = P3 - P1 + P2
+    //   update:  A = Ur Vr,    B = Ui Vi,    C = (Ur + Ui)(Vr + Vi)      =>  qr += A - B,   qi += C - A - B
+    // P1..P3 are accumulated over a whole pass and turned into W at its end.
+    double P1[8][2], P2[8][2], P3[8][2], Ur[8][2], Ui[8][2];
 #pragma unroll
     for (int i = 0; i < 8; ++i)
 #pragma unroll
-        for (int e = 0; e < 2; ++e) Wr[i][e] = Wi[i][e] = Ur[i][e] = Ui[i][e] = nUi[i][e] = 0.0;
+        for (int e = 0; e < 2; ++e) P1[i][e] = P2[i][e] = P3[i][e] = Ur[i][e] = Ui[i][e] = 0.0;
 
     int64_t P = npb, g = b2f_glo(npb, a.nbw, 2);
     while (P >= 0) {
@@ -210,24 +216,29 @@ __device__ __forceinline__ void b2fz_consume(const B2fArgs &a, unsigned char *sm
         qst_out = (qst_out + 1 == NSQ) ? 0 : qst_out + 1;
 
         if (has_upd) {
-            // --- q^T += U^T V_P^T: chunk (i, e): k-slot r = reflector 8i + 2r + e; four accumulator chains
-            double Zr[2] = {0.0, 0.0}, Zi[2] = {0.0, 0.0};
+            // --- q^T += U^T V_P^T: chunk (i, e): k-slot r = reflector 8i + 2r + e; A, B, C in two sets (e = 0 / 1):
+            //     six independent accumulator chains
+            double A[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, B[2][2] = {{0.0, 0.0}, {0.0, 0.0}}, Cc[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
             const double *bp = pa + (2 * r) * S + 2 * gq;
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const double2 b = *reinterpret_cast<const double2 *>(bp + (8 * i + e) * S);
-                    dmma884(Yr[0], Yr[1], Ur[i][e], b.x, Yr[0], Yr[1]);
-                    dmma884(Yi[0], Yi[1], Ur[i][e], b.y, Yi[0], Yi[1]);
-                    dmma884(Zr[0], Zr[1], nUi[i][e], b.y, Zr[0], Zr[1]);
-                    dmma884(Zi[0], Zi[1], Ui[i][e], b.x, Zi[0], Zi[1]);
+                    dmma884(A[e][0], A[e][1], Ur[i][e], b.x, A[e][0], A[e][1]);
+                    dmma884(B[e][0], B[e][1], Ui[i][e], b.y, B[e][0], B[e][1]);
+                    dmma884(Cc[e][0], Cc[e][1], Ur[i][e] + Ui[i][e], b.x + b.y, Cc[e][0], Cc[e][1]);
                 }
-            Yr[0] += Zr[0], Yr[1] += Zr[1], Yi[0] += Zi[0], Yi[1] += Zi[1];
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                const double pa_ = A[0][c] + A[1][c], pb_ = B[0][c] + B[1][c], pc_ = Cc[0][c] + Cc[1][c];
+                Yr[c] += pa_ - pb_;
+                Yi[c] += (pc_ - pa_) - pb_;
+            }
         }
         if (has_dot) {
             // --- W^T += q^T conj(V_{P-1}): k-chunk e: k-slot r = row 2r + e; n-tile i = reflectors 8i + n
-            const double nYr[2] = {-Yr[0], -Yr[1]};
+            const double Ys[2] = {Yr[0] + Yi[0], Yr[1] + Yi[1]};
             const double *bp = pb + gq * S + 4 * r;
 #pragma unroll
             for (int i = 0; i < 8; i += 2) {
@@ -240,15 +251,9 @@ __device__ __forceinline__ void b2fz_consume(const B2fArgs &a, unsigned char *sm
                 for (int e = 0; e < 2; ++e)
 #pragma unroll
                     for (int d = 0; d < 2; ++d) {
-                        dmma884(Wr[i + d][0], Wr[i + d][1], Yr[e], b[d][e].x, Wr[i + d][0], Wr[i + d][1]);
-                        dmma884(Wi[i + d][0], Wi[i + d][1], Yi[e], b[d][e].x, Wi[i + d][0], Wi[i + d][1]);
-                    }
-#pragma unroll
-                for (int e = 0; e < 2; ++e)
-#pragma unroll
-                    for (int d = 0; d < 2; ++d) {
-                        dmma884(Wr[i + d][0], Wr[i + d][1], Yi[e], b[d][e].y, Wr[i + d][0], Wr[i + d][1]);
-                        dmma884(Wi[i + d][0], Wi[i + d][1], nYr[e], b[d][e].y, Wi[i + d][0], Wi[i + d][1]);
+                        dmma884(P1[i + d][0], P1[i + d][1], Yr[e], b[d][e].x, P1[i + d][0], P1[i + d][1]);
+                        dmma884(P2[i + d][0], P2[i + d][1], Yi[e], b[d][e].y, P2[i + d][0], P2[i + d][1]);
+                        dmma884(P3[i + d][0], P3[i + d][1], Ys[e], b[d][e].x - b[d][e].y, P3[i + d][0], P3[i + d][1]);
                     }
             }
         }
@@ -265,6 +270,15 @@ __device__ __forceinline__ void b2fz_consume(const B2fArgs &a, unsigned char *sm
             // --- end of pass: U^T = W^T (-T_{P-1})^T.  n-tile i' = reflectors 8i' + n; k chunk (i, e): k-slot r =
             //     reflector 8i + 2r + e; B[k][n] = T'[8i' + n][k], zero for k-tiles i < i' (T upper triangular)
             const double *tp = a.tneg + ((P - 1) * (NB * NB) + gq * NB + 2 * r) * 2;
+            // W from the three accumulators, in place: Wr -> P1, Wi -> P3
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const double p1 = P1[i][e], p2 = P2[i][e];
+                    P1[i][e] = p1 + p2;
+                    P3[i][e] = (P3[i][e] - p1) + p2;
+                }
 #pragma unroll
             for (int ip = 0; ip < 8; ++ip) {
                 double cr[2] = {0.0, 0.0}, ci[2] = {0.0, 0.0}, dr[2] = {0.0, 0.0}, di[2] = {0.0, 0.0};
@@ -273,21 +287,20 @@ __device__ __forceinline__ void b2fz_consume(const B2fArgs &a, unsigned char *sm
 #pragma unroll
                     for (int e = 0; e < 2; ++e) {
                         const double2 t = __ldg(reinterpret_cast<const double2 *>(tp + (8 * ip * NB + 8 * i + e) * 2));
-                        dmma884(cr[0], cr[1], Wr[i][e], t.x, cr[0], cr[1]);
-                        dmma884(ci[0], ci[1], Wr[i][e], t.y, ci[0], ci[1]);
-                        dmma884(dr[0], dr[1], Wi[i][e], -t.y, dr[0], dr[1]);
-                        dmma884(di[0], di[1], Wi[i][e], t.x, di[0], di[1]);
+                        dmma884(cr[0], cr[1], P1[i][e], t.x, cr[0], cr[1]);
+                        dmma884(ci[0], ci[1], P1[i][e], t.y, ci[0], ci[1]);
+                        dmma884(dr[0], dr[1], P3[i][e], -t.y, dr[0], dr[1]);
+                        dmma884(di[0], di[1], P3[i][e], t.x, di[0], di[1]);
                     }
                 }
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     Ur[ip][e] = cr[e] + dr[e];
                     Ui[ip][e] = ci[e] + di[e];
-                    nUi[ip][e] = -Ui[ip][e];
                 }
             }
 #pragma unroll
-            for (int i = 0; i < 8; ++i) Wr[i][0] = Wr[i][1] = Wi[i][0] = Wi[i][1] = 0.0;
+            for (int i = 0; i < 8; ++i) P1[i][0] = P1[i][1] = P2[i][0] = P2[i][1] = P3[i][0] = P3[i][1] = 0.0;
         }
         if (g < ghi) {
             ++g;

@@ -281,36 +281,43 @@ __device__ __forceinline__ void wyz_consume(const WyArgs &a, unsigned char *smem
             const double *va = stage + C::VA_OFF + (gq * C::SA + 2 * r) * 2;   // + (8t + e) * 2
             const double *vb = stage + C::YB_OFF + (gq * C::SB + 2 * r) * 2;   // + 8t * SB * 2 + e * 2
 
-            // --- D^T = x^T conj(V): A1 = xr Vr, A2 = xi Vi, A3 = xi Vr, A4 = xr Vi
-            double A1[NG][2], A2[NG][2], A3[NG][2], A4[NG][2];
+            // --- D^T = x^T conj(V) with three real products instead of four (the 3M form of a complex product):
+            //     P1 = xr Vr, P2 = xi Vi, P3 = (xr + xi)(Vr - Vi)  =>  Dr = P1 + P2, Di = P3 - P1 + P2.
+            //     The two operand sums are one DADD each per k-chunk (same FP64 pipe: 2 cycles against the 16 of
+            //     the DMMA they replace); normwise the rounding error is that of the four-product form.
+            //     Two accumulator sets (e = 0 / 1): six independent DMMA chains per slab.
+            double P1[NG][2][2], P2[NG][2][2], P3[NG][2][2];
 #pragma unroll
             for (int g = 0; g < NG; ++g)
-                A1[g][0] = A1[g][1] = A2[g][0] = A2[g][1] = A3[g][0] = A3[g][1] = A4[g][0] = A4[g][1] = 0.0;
+#pragma unroll
+                for (int e = 0; e < 2; ++e)
+                    P1[g][e][0] = P1[g][e][1] = P2[g][e][0] = P2[g][e][1] = P3[g][e][0] = P3[g][e][1] = 0.0;
 #pragma unroll
             for (int tt = 0; tt < NT; ++tt) {
                 const int t = (tt + 1) % NT;
 #pragma unroll
                 for (int e = 0; e < 2; ++e) {
                     const double2 v2 = *reinterpret_cast<const double2 *>(va + (8 * t + e) * 2);
+                    const double vd = v2.x - v2.y;
 #pragma unroll
                     for (int g = 0; g < NG; ++g) {
                         const double xr = t ? Xr[g][t][e] : T0[g][e], xi = t ? Xi[g][t][e] : T0[g][2 + e];
-                        dmma884(A1[g][0], A1[g][1], xr, v2.x, A1[g][0], A1[g][1]);
-                        dmma884(A2[g][0], A2[g][1], xi, v2.y, A2[g][0], A2[g][1]);
-                        dmma884(A3[g][0], A3[g][1], xi, v2.x, A3[g][0], A3[g][1]);
-                        dmma884(A4[g][0], A4[g][1], xr, v2.y, A4[g][0], A4[g][1]);
+                        dmma884(P1[g][e][0], P1[g][e][1], xr, v2.x, P1[g][e][0], P1[g][e][1]);
+                        dmma884(P2[g][e][0], P2[g][e][1], xi, v2.y, P2[g][e][0], P2[g][e][1]);
+                        dmma884(P3[g][e][0], P3[g][e][1], xr + xi, vd, P3[g][e][0], P3[g][e][1]);
                     }
                 }
             }
-            // --- E^T = D^T (T is folded into YB = V (-T)): Er = A1 + A2, Ei = A3 - A4
+            // --- E^T = D^T (T is folded into YB = V (-T)): Er = P1 + P2, Ei = P3 - P1 + P2
             double Er[NG][2], Ei[NG][2], nEi[NG][2];
 #pragma unroll
             for (int g = 0; g < NG; ++g)
 #pragma unroll
-                for (int e = 0; e < 2; ++e) {
-                    Er[g][e] = A1[g][e] + A2[g][e];
-                    Ei[g][e] = A3[g][e] - A4[g][e];
-                    nEi[g][e] = A4[g][e] - A3[g][e];
+                for (int c = 0; c < 2; ++c) {
+                    const double p1 = P1[g][0][c] + P1[g][1][c], p2 = P2[g][0][c] + P2[g][1][c], p3 = P3[g][0][c] + P3[g][1][c];
+                    Er[g][c] = p1 + p2;
+                    Ei[g][c] = (p3 - p1) + p2;
+                    nEi[g][c] = -Ei[g][c];
                 }
             // --- x^T += E^T Y^T: xr += Er Yr - Ei Yi, xi += Er Yi + Ei Yr; tile t -> registers of t+1
 #pragma unroll
