@@ -21,11 +21,11 @@
 //    Lane (gq, r) = (lane / 4, lane % 4) holds rows 4r .. 4r+3 of column gq of a 16-row group (32
 //    contiguous bytes; the four lanes of a column cover one 128-byte line).
 //  * V tiles (16 rows x 64 reflectors of block P and of block P-1) are staged by the warps in turn
-//    with 16-byte cp.async (zero fill beyond N / Nv) into an 8-stage shared-memory ring (staged 4 items ahead)
+//    with 16-byte cp.async (zero fill beyond N / Nv) into a 4-stage shared-memory ring
 //    [reflector][18 doubles]: the row stride 18 makes both B-fragment access patterns (LDS.128)
 //    bank-conflict free.  Completion on mbarriers, no CTA barrier in the loop.
 //  * A warp owns 1 or 2 slabs of 8 columns for ALL passes: W and U (2 x 16 doubles per slab) live in
-//    registers.  Its rows of q arrive through a private 4-stage shared-memory ring filled by its own
+//    registers.  Its rows of q arrive through a private 6-stage shared-memory ring filled by its own
 //    cp.async copies four items ahead (no register is tied up by a load in flight, and no scoreboard is
 //    shared between the q stream and the B-fragment loads); updated rows go back to global memory
 //    straight from the C fragments.  CTAs never communicate; a CTA walks its slabs in rounds of up to 16.
@@ -43,12 +43,12 @@ struct B2fCfg {
     static constexpr int S = 18;                      // smem row stride per reflector (doubles): S/2 odd
     static constexpr int PANEL = NB * S;              // doubles per panel tile
     static constexpr int STAGE_DOUBLES = 2 * PANEL;   // panel 0: block P (update), panel 1: block P-1 (dot)
-    static constexpr int NS = 8, LGNS = 3, LAG = 4;   // V ring (shared by the CTA): staged 4 items ahead
+    static constexpr int NS = 4, LGNS = 2, LAG = 2;   // V ring (shared by the CTA); 8 stages / 4 ahead measured the same
     static constexpr int NW = 8;                      // warps per CTA
     static constexpr int NGMAX = 2;                   // slabs per warp
     static constexpr int QS = 18;                     // q tile: [column][QS doubles], QS/2 odd
     static constexpr int QTILE = 8 * NGMAX * QS;      // doubles per q tile (one warp, one item)
-    static constexpr int NSQ = 4, DQ = 3;             // q ring per warp: stages, items fetched ahead (DQ <= 4, see b2f_consume)
+    static constexpr int NSQ = 6, DQ = 4;             // q ring per warp: stages, items fetched ahead (DQ <= 4, see b2f_consume)
     static constexpr int OFF_Q = NS * STAGE_DOUBLES * 8;
     static constexpr int OFF_BAR = OFF_Q + NW * NSQ * QTILE * 8;
     static constexpr int SMEM_BYTES = OFF_BAR + 2 * NS * 8;
