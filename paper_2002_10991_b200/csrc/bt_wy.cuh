@@ -579,6 +579,19 @@ inline int wy_pick_P_real(int64_t nslab, int64_t K0, int nsm, int ngmax, int max
     return (ok(2) && wy_smsp_load(2, n) * 1.03 < wy_smsp_load(1, n)) ? 2 : 1;
 }
 
+// Complex kernel (P <= 2): up to 4 slabs per SM the rule of round 1 (one slab per warp, two warps per slab:
+// 18.7 -> 25.4 TFLOP/s on config 3); above that, while the P = 2 launch still fits in one wave
+// (n <= 4 ngmax), P = 2 when it lowers the busiest sub-partition.
+inline int wy_pick_P_cplx(int64_t nslab, int64_t K0, int nsm, int ngmax, int maxP)
+{
+    const int base = wy_pick_P(nslab, K0, nsm, 8, maxP);
+    if (base > 1) return base;
+    const int64_t grid = nslab < nsm ? nslab : nsm;
+    const int64_t n = (nslab + grid - 1) / grid;
+    if (maxP >= 2 && 8 <= K0 && n > 4 && n <= 4 * (int64_t)ngmax && wy_smsp_load(2, n) * 1.03 < wy_smsp_load(1, n)) return 2;
+    return 1;
+}
+
 // launch plan of the main kernel (pure host arithmetic; exported as elpa2_bt_plan for the CPU tests)
 struct WyPlan {
     int64_t grid;        // CTAs
@@ -601,10 +614,10 @@ inline WyPlan wy_plan(bool cplx, int nbw, int64_t N, int64_t nev, int nsm, int f
     if (force_P > maxP) force_P = maxP;
     pl.P = many_warps ? 4
            : force_P > 0 ? force_P
-           : cplx ? wy_pick_P(pl.nslab, K0, nsm, 8, maxP)
+           : cplx ? wy_pick_P_cplx(pl.nslab, K0, nsm, ngmax8, maxP)
                   : wy_pick_P_real(pl.nslab, K0, nsm, ngmax8, maxP);
-    // (the complex kernel and the 16-warp build walk one slab per warp in chain-parallel mode)
-    pl.per_cta = (int64_t)(pl.nwarps / pl.P) * ((many_warps || (cplx && pl.P > 1)) ? 1 : ngmax8);
+    // (the 16-warp build walks one slab per warp)
+    pl.per_cta = (int64_t)(pl.nwarps / pl.P) * (many_warps ? 1 : ngmax8);
     const int64_t waves = (pl.nslab + nsm * pl.per_cta - 1) / (nsm * pl.per_cta);
     pl.grid = nsm * waves;                            // a multiple of the SM count ...
     if (pl.grid > pl.nslab) pl.grid = pl.nslab;       // ... unless there are fewer slabs than that

@@ -424,7 +424,8 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     const int64_t nslab = (a.nev + 7) >> 3;
     const int64_t slab0 = nslab * blockIdx.x / gridDim.x;
     const int nmine = (int)(nslab * (blockIdx.x + 1) / gridDim.x - slab0);
-    const int nact = nmine < NW ? nmine : NW;
+    const int nslot = NW / (a.P > 1 ? a.P : 1);
+    const int nact = nmine < nslot ? nmine : nslot;    // members of a ring (P = 1: active warps)
 
     for (int i = threadIdx.x; i < C::OFF_BAR / 8; i += blockDim.x) ring[i] = 0.0;
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -438,9 +439,16 @@ __global__ void __launch_bounds__(256, 1) bt_wyz_kernel(const WyArgs a)
     __syncthreads();
 
     if (!RG && a.P > 1) {
-        const int grp = warp % a.P, member = warp / a.P;
-        if (member >= nmine) return;
-        wyz_consume<C, 1, true, false>(a, smem, lane, grp, member, nmine, (slab0 + member) << 3, slab0 + member);
+        // chain-parallel: NW / P groups of P warps; a group takes nmine / (NW / P) slabs (+1 for the first ones)
+        const int grp = warp % a.P, member = warp / a.P, nm = NW / a.P;
+        const int base = nmine / nm, extra = nmine % nm;
+        const int ng = base + (member < extra ? 1 : 0);
+        const int64_t wslab0 = slab0 + (int64_t)member * base + (member < extra ? member : extra);
+        if (ng == 0) return;
+        if (NGMAX >= 2 && ng == 2)
+            wyz_consume<C, (NGMAX >= 2 ? 2 : 1), true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
+        else
+            wyz_consume<C, 1, true, false>(a, smem, lane, grp, member, nact, wslab0 << 3, wslab0);
         return;
     }
     const int base = nmine / NW, extra = nmine % NW;

@@ -160,7 +160,9 @@ def test_launch_plan_balances_sub_partitions_for_partial_spectra():
     assert binding.plan(False, N, 128, 148 * 8 * 4, 148)["P"] == 4
     assert binding.plan(False, N, 128, 148 * 8 * 7, 148)["P"] == 2
     assert binding.plan(False, N, 256, 148 * 8 * 3, 148)["P"] == 2      # 4 ring stages: P <= 2
-    assert binding.plan(True, 16384, 128, 8192, 148)["P"] == 1          # complex: unchanged
+    assert binding.plan(True, 16384, 128, 8192, 148)["P"] == 1          # complex nbw 128: one slab per warp, 7 per SM
+    assert binding.plan(True, 8192, 64, 148 * 8 * 6, 148)["P"] == 2     # complex nbw 64, 6 slabs per SM: 2 + 2 + 1 + 1 on pairs
+    assert binding.plan(True, 8192, 64, 148 * 8 * 7, 148)["P"] == 1
 
 
 def test_launch_plan_invariants():

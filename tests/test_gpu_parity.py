@@ -109,6 +109,21 @@ def test_partial_spectrum_plans(nbw, n):
     _check(N, nbw, nev, False)
 
 
+@pytest.mark.parametrize("nbw,n", [(32, 5), (64, 6), (64, 8)])
+def test_partial_spectrum_plans_complex(nbw, n):
+    # complex: P = 2 with two slabs per group of warps (5-8 slabs per CTA)
+    from paper_2002_10991_b200 import binding
+
+    N, nev = 17 * nbw + 1, 148 * 8 * n - 3
+    assert binding.plan(True, N, nbw, nev, 148)["P"] == (2 if n < 8 else 1)
+    _check(N, nbw, nev, True)
+    old = binding.set_chain_parallel(2)                 # forced: also the shapes the plan leaves at P = 1
+    try:
+        _check(N, nbw, nev, True, seed=1)
+    finally:
+        binding.set_chain_parallel(old)
+
+
 @pytest.mark.parametrize("cplx", [False, True])
 def test_more_columns_than_one_wave(cplx):
     # more slabs than 148 CTAs x 8 warps x NGMAX: the grid becomes a multiple of the SM count > 1
