@@ -196,20 +196,26 @@ def run_reference(args, rank: int) -> None:
     lengths = np.minimum(nbw, N - 1 - s_of_g - k_of_g * nbw)
     hv, ht = si.synthetic_reflectors(lengths, nbw, seed_r, cplx, "cpu")
     hv, ht = hv.numpy(), ht.numpy()
+    single = args.dtype == "f32"
+    if single:                                         # the FP32 oracle on the same stream rounded to float
+        f32 = np.complex64 if cplx else np.float32
+        hv, ht = hv.astype(f32), ht.astype(f32)
     ncols = oracle_sample_cols(cplx, N, cores)
     times = []
     for i in range(args.warmup + args.steps):
-        t, _ = oracle_sample_run(cplx, N, nbw, hv, ht, ncols, seed_x + i)
+        t, _ = oracle_sample_run(cplx, N, nbw, hv, ht, ncols, seed_x + i, single)
         if i >= args.warmup:
             times.append(t)
     total = sum(times)
     gflops = model_flops(cplx, N, ncols) * len(times) / total / 1e9
     sample = f"{ncols} seeded N(0,1) columns of {nev} per step (columns are independent, PAPER.md:134)"
     print(json.dumps({
-        "impl": "reference", "metric": METRIC, "value": gflops, "unit": "GFLOP/s", "n_gpus": args.gpus,
+        "impl": "reference", "metric": METRIC.replace("FP64", "FP32") if single else METRIC, "value": gflops,
+        "unit": "GFLOP/s", "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-        "data": "synthetic", "config": {"workload": workload_name(args.config), "reflectors":
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": args.dtype,
+        "data": "synthetic", "config": {"workload": workload_name(args.config) + (" [FP32 arithmetic]" if single else ""),
+                                        "reflectors":
                                         "synthetic unitary stream (host-generated)"},
         "cpu_baseline": {"value": gflops, "unit": "GFLOP/s", "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": gflops, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
