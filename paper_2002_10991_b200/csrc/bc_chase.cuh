@@ -375,15 +375,19 @@ __device__ __forceinline__ bool bc_step_smem(const int64_t N, const int64_t s, c
             }
             w2[i] = dot;
         }
-        asm volatile("bar.sync 1, 64;" ::: "memory");
-        for (int j = t64; j < L; j += 64)
-#pragma unroll 4
-            for (int i = j; i < L; ++i) {
+    }
+    __syncthreads();
+    // (ii), last phase: D' = M - tau w2 v^T is element-wise -- all threads (its owner group alone, one thread per
+    // column with up to L elements each, was the longest chain of the step)
+    if (tau != 0.0) {
+        const int ty = tid / NBW, i = tid - ty * NBW, RY = nt / NBW;
+        for (int j = ty; j < L; j += RY)
+            if (i >= j && i < L) {
                 const double m = __dsub_rn(BS(i, nA + j), __dmul_rn(__dmul_rn(tau, v[i]), p[j]));
                 BS(i, nA + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
             }
+        __syncthreads();
     }
-    __syncthreads();
 #undef BS
     // --- stage out (block (iii) stays behind if the next step takes it from S): a warp per column, two
     //     columns at a time through registers, so that the shared-memory loads of both are in flight together
