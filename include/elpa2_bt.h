@@ -161,6 +161,20 @@ int elpa2_trans_ev_band_to_full_d(int64_t N, int nbw, int64_t nev, const double 
 int elpa2_trans_ev_band_to_full_z(int64_t N, int nbw, int64_t nev, const void *hv, int64_t ldv,
                                   const void *tau, void *q, int64_t ldq, void *stream);
 
+/* Allocation-free variant of elpa2_trans_ev_band_to_full_d for callers that cannot allocate (CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): same operation, same arguments, same
+ * kernels and results, but the -T factors go into a static 16 MiB device array inside the library
+ * (elpa2_noalloc_scratch_bytes(); every GPU that loads the library holds it until the process exits)
+ * instead of the stream-ordered pool.  The call issues no cudaMalloc / cudaFree / cudaMallocAsync and no
+ * allocating library routine.  Limit: 32 KB per block of 64 reflectors, i.e. N - nbw - 1 <= 32768; a larger
+ * problem returns -20 and launches nothing.  ALL calls share the one array (per device): calls that overlap
+ * on the GPU -- two streams, or two threads -- race on it; issue them on one stream or synchronise between
+ * them.  The array keeps the last call's contents; each call's prepass overwrites every entry it reads,
+ * so nothing has to be cleared.  Other return codes as elpa2_trans_ev_band_to_full_d. */
+int elpa2_trans_ev_band_to_full_noalloc_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv,
+                                          const double *tau, double *q, int64_t ldq, void *stream);
+int64_t elpa2_noalloc_scratch_bytes(void);
+
 /* Same operation with HOST buffers (pageable or pinned), synchronous: H2D of hv, tau and q, the two
  * kernels, D2H of q (what bench.py --step 6e reports as e2e).  Device scratch cached as for
  * elpa2_trans_ev_tridi_to_band_host.  Argument positions: is_complex=1, N=2, nbw=3, nev=4, hv=5, ldv=6,

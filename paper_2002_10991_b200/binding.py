@@ -26,6 +26,7 @@ EXPORTS = (
     "elpa2_trans_ev_band_to_full_host", "elpa2_bt_set_chain_parallel",
     "elpa2_trans_ev_tridi_to_band_s", "elpa2_trans_ev_tridi_to_band_c", "elpa2_trans_ev_tridi_to_band_host32",
     "elpa2_trans_ev_tridi_to_band_rows_d", "elpa2_trans_ev_tridi_to_band_rows_z",
+    "elpa2_trans_ev_band_to_full_noalloc_d", "elpa2_noalloc_scratch_bytes",
 )
 
 
@@ -64,7 +65,9 @@ def lib() -> ctypes.CDLL:
         for nm in ("elpa2_bulge_chase_d", "elpa2_bulge_chase_z"):
             getattr(L, nm).argtypes = [i64, i32, vp, vp, vp, vp, vp, vp]
             getattr(L, nm).restype = i32
-        for nm in ("elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z"):
+        L.elpa2_noalloc_scratch_bytes.argtypes = []
+        L.elpa2_noalloc_scratch_bytes.restype = i64
+        for nm in ("elpa2_trans_ev_band_to_full_d", "elpa2_trans_ev_band_to_full_z", "elpa2_trans_ev_band_to_full_noalloc_d"):
             getattr(L, nm).argtypes = [i64, i32, i64, vp, i64, vp, vp, i64, vp]
             getattr(L, nm).restype = i32
         L.elpa2_trans_ev_band_to_full_host.argtypes = [i32, i64, i32, i64, vp, i64, vp, vp, i64]
@@ -99,6 +102,8 @@ class Elpa2BtError(RuntimeError):
     def __init__(self, rc: int):
         self.rc = rc
         what = f"argument {-rc} invalid" if rc < 0 else f"cudaError_t {rc}"
+        if rc == -20:
+            what = "the problem needs more scratch than the static no-alloc array holds (elpa2_noalloc_scratch_bytes)"
         super().__init__(f"elpa2_trans_ev_tridi_to_band failed: {what}")
 
 
@@ -243,6 +248,36 @@ def trans_ev_tridi_to_band_rows(N: int, nbw: int, hh_v, hh_tau, q_local, row0: i
     fn = lib().elpa2_trans_ev_tridi_to_band_rows_z if cplx else lib().elpa2_trans_ev_tridi_to_band_rows_d
     rc = fn(N, nbw, nev, hh_v.data_ptr(), hh_tau.data_ptr(), q_local.data_ptr(), ldq, row0, nown, nloc, kb, ke,
             _stream_ptr(stream))
+    if rc != 0:
+        raise Elpa2BtError(rc)
+
+
+def noalloc_scratch_bytes() -> int:
+    return int(lib().elpa2_noalloc_scratch_bytes())
+
+
+def trans_ev_band_to_full_noalloc(N: int, nbw: int, hv, tau, q, stream=None) -> None:
+    """``elpa2_trans_ev_band_to_full_noalloc_d``: Eq. 6e, real FP64, without any allocation -- the scratch is a
+    static 16 MiB device array inside the library (N - nbw - 1 <= 32768, else Elpa2BtError with rc -20).  All
+    calls share that array: calls that overlap on the GPU race.  Arguments as ``trans_ev_band_to_full``."""
+    import torch
+
+    if not (q.is_cuda and hv.is_cuda and tau.is_cuda):
+        raise ValueError("device tensors required")
+    if q.dtype != torch.float64 or hv.dtype != q.dtype or tau.dtype != q.dtype:
+        raise ValueError("float64 throughout")
+    Nv = max(N - nbw - 1, 0)
+    if q.dim() != 2 or q.shape[0] != N or (N > 1 and q.stride(0) != 1):
+        raise ValueError("q must be (N, nev) column-major")
+    nev = q.shape[1]
+    ldq = q.stride(1) if nev > 1 else max(N, 1)
+    if Nv > 0 and (tuple(hv.shape) != (N, Nv) or hv.stride(0) != 1 or tuple(tau.shape) != (Nv,) or not tau.is_contiguous()):
+        raise ValueError(f"hv must be ({N}, {Nv}) column-major and tau ({Nv},)")
+    ldv = hv.stride(1) if Nv > 1 else max(N + (N & 1), 2)
+    if not (hv.device == q.device and tau.device == q.device and torch.cuda.current_device() == q.device.index):
+        raise ValueError("hv, tau and q must live on the current CUDA device")
+    rc = lib().elpa2_trans_ev_band_to_full_noalloc_d(N, nbw, nev, hv.data_ptr(), ldv, tau.data_ptr(), q.data_ptr(), ldq,
+                                                     _stream_ptr(stream))
     if rc != 0:
         raise Elpa2BtError(rc)
 

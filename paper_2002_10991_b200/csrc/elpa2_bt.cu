@@ -324,6 +324,33 @@ struct Scratch {
     }
 } g_sv, g_st, g_sq;
 
+// ---- allocation-free entry point (elpa2_trans_ev_band_to_full_noalloc_d) ------------------------------------
+// Its scratch -- the -T factors of the Eq. 6e blocks, 32 KB per block of 64 reflectors -- lives in this
+// file-scope device array instead of the stream-ordered pool: 16 MiB, held by every GPU that loads the
+// library until the process exits.  In host code the array's NAME is a host-side stand-in, not a device
+// address: the address comes from cudaGetSymbolAddress, once per device with that device current.
+constexpr size_t NOALLOC_SCRATCH_BYTES = (size_t)16 << 20;
+static __device__ __align__(256) double g_noalloc_scratch[NOALLOC_SCRATCH_BYTES / sizeof(double)];
+std::mutex g_noalloc_mu;
+void *g_noalloc_ptr[MAX_DEV] = {};      // device address of g_noalloc_scratch, per device
+
+cudaError_t noalloc_scratch_ptr(void **out)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEV) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_noalloc_mu);
+    if (!g_noalloc_ptr[dev]) {
+        void *p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess) return e;
+        g_noalloc_ptr[dev] = p;
+    }
+    *out = g_noalloc_ptr[dev];
+    return cudaSuccess;
+}
+
 }  // namespace
 
 extern "C" {
@@ -566,6 +593,33 @@ int elpa2_trans_ev_band_to_full_z(int64_t N, int nbw, int64_t nev, const void *h
     const cudaError_t e2 = cudaFreeAsync(scratch, st);
     if (e != cudaSuccess) return (int)e;
     if (e2 != cudaSuccess) return (int)e2;
+    g_last_launches = 2;
+    return 0;
+}
+
+int64_t elpa2_noalloc_scratch_bytes(void) { return (int64_t)NOALLOC_SCRATCH_BYTES; }
+
+int elpa2_trans_ev_band_to_full_noalloc_d(int64_t N, int nbw, int64_t nev, const double *hv, int64_t ldv,
+                                          const double *tau, double *q, int64_t ldq, void *stream)
+{
+    if (N < 0) return -1;
+    if (nbw < 16 || (nbw & 15) != 0) return -2;
+    if (nev < 0) return -3;
+    g_last_launches = 0;
+    if (N - nbw - 1 <= 0 || nev == 0) return 0;          // no reflector: P = I
+    if (b2f_scratch_bytes(N, nbw) > NOALLOC_SCRATCH_BYTES) return -20;   // more blocks than the static scratch holds
+    if (!hv || ((uintptr_t)hv & 15) != 0) return -4;
+    if (ldv < N || (ldv & 1) != 0) return -5;
+    if (!tau || ((uintptr_t)tau & 7) != 0) return -6;
+    if (!q || ((uintptr_t)q & 7) != 0) return -7;
+    if (ldq < N) return -8;
+    void *scratch = nullptr;
+    cudaError_t e = noalloc_scratch_ptr(&scratch);
+    if (e != cudaSuccess) return (int)e;
+    const int align16 = (((uintptr_t)q & 15) == 0 && (ldq & 1) == 0) ? 1 : 0;
+    // the prepass overwrites every entry of the -T factors this call reads: nothing has to start at zero
+    e = launch_b2f(N, nbw, nev, hv, ldv, tau, q, ldq, align16, sm_count(), scratch, (cudaStream_t)stream);
+    if (e != cudaSuccess) return (int)e;
     g_last_launches = 2;
     return 0;
 }
