@@ -510,8 +510,16 @@ template <int NBW>
 __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t s, const int64_t k, zc *__restrict__ ab,
                                                  zc *__restrict__ hh_v, zc *__restrict__ hh_tau, zc *v, zc *p, zc *w2,
                                                  zc *zsc, double *dsc, uint32_t *head_mine = nullptr,
-                                                 const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
+                                                 const uint32_t *head_prev = nullptr, const uint32_t need_head = 0,
+                                                 zc *TD = nullptr)
 {
+    // TD != nullptr (persistent kernel, 384 threads): shared memory for the lower triangle of the diagonal
+    // block, packed by columns (column j: rows j .. NBW-1 at TD + toff(j)), followed by NBW dot products.
+    // Block (ii) -- three dependent phases, the longest chain of the step -- then runs out of shared
+    // memory, and the element-wise second halves of (i) and (ii) run on all threads with coalesced
+    // accesses after the groups have met.  Same operations in the same order within every sum.
+    constexpr int TRI = NBW * (NBW + 1) / 2;
+    auto toff = [](int j) { return j * NBW - ((j * (j - 1)) >> 1); };
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     constexpr int64_t ldab = 2 * NBW + 1;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -530,6 +538,16 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
             if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
         }
         return;
+    }
+    if (TD) {
+        // the diagonal block was last written by steps that are finished (done flags): fetch it while the
+        // generator runs; a warp per column, lanes along its contiguous rows
+        for (int j = tid >> 5; j < L; j += nt >> 5) {
+            const zc *src = &BC_Z(r0 + j, r0 + j);
+            zc *dst = TD + toff(j);
+            for (int i = tid & 31; i < L - j; i += 32) cp_async16(smem_u32(dst + i), src + i, 16u);
+        }
+        cp_async_commit();
     }
     // --- Householder generator (R2, R7): beta real, tau = ((beta - Re a)/beta, -Im a/beta), v = x/(alpha - beta)
     if (tid < L) p[tid] = BC_Z(r0 + tid, c);
@@ -566,7 +584,74 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
         hh_tau[g] = tau;
         if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
+    if (TD) {
+        cp_async_wait_all();
+        __syncthreads();
+    }
     if (ident) return;
+    if (TD) {
+        const int grp = tid >> 7, t0 = tid & 127;
+        zc *dA = TD + TRI;
+#define DZ(i, j) (((i) >= (j)) ? TD[toff(j) + (i) - (j)] : zconj(TD[toff(i) + (j) - (i)]))
+        if (grp == 0) {
+            // --- (i), first half: the dot products v^H A, one thread per column
+            for (int64_t j = c + 1 + t0; j < r0; j += 128) {
+                zc dot = {0.0, 0.0};
+                for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), BC_Z(r0 + i, j)));
+                dA[j - (c + 1)] = dot;
+            }
+        } else if (grp == 1) {
+            // --- (iii) E <- E H = E - tau (E v) v^H, one thread per row (coalesced both ways)
+            int64_t r2 = r1 + NBW;
+            if (r2 > N - 1) r2 = N - 1;
+            for (int64_t i = r1 + 1 + t0; i <= r2; i += 128) {
+                if (need_head && i == r2) {      // the corner is the head element of step (s-1, k+2): wait for its beta
+                    uint32_t h;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                    } while (h < need_head);
+                }
+                zc dot = {0.0, 0.0};
+                for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
+                for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
+            }
+        } else {
+            // --- (ii), first two phases, out of shared memory: p = v^H D;  w2 = (D - conj(tau) v p) v
+            for (int j = t0; j < L; j += 128) {
+                zc dot = {0.0, 0.0};
+#pragma unroll 4
+                for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), DZ(i, j)));
+                p[j] = dot;
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int i = t0; i < L; i += 128) {
+                zc dot = {0.0, 0.0};
+#pragma unroll 4
+                for (int j = 0; j < L; ++j) {
+                    const zc m = zsub(DZ(i, j), zmul(zmul(ctau, v[i]), p[j]));
+                    dot = zadd(dot, zmul(m, v[j]));
+                }
+                w2[i] = dot;
+            }
+        }
+        __syncthreads();
+        // --- second halves, element-wise, all threads: thread = row i (contiguous in memory), ty strides the columns
+        {
+            const int ty = tid >> 7, i = tid & 127;
+            if (i < L) {
+                for (int64_t j = c + 1 + ty; j < r0; j += 3)
+                    BC_Z(r0 + i, j) = zsub(BC_Z(r0 + i, j), zmul(zmul(ctau, v[i]), dA[j - (c + 1)]));
+                for (int j = ty; j <= i; j += 3) {
+                    const zc m = zsub(TD[toff(j) + i - j], zmul(zmul(ctau, v[i]), p[j]));
+                    zc r = zsub(m, zmul(zmul(tau, w2[i]), zconj(v[j])));
+                    if (i == j) r.im = 0.0;              // a Hermitian diagonal is real
+                    BC_Z(r0 + i, r0 + j) = r;
+                }
+            }
+        }
+#undef DZ
+        return;
+    }
     // With 384 threads (persistent kernel) three groups of 128 run the disjoint blocks (i), (iii), (ii) side
     // by side ((ii) synchronises on a named barrier of its own); with fewer threads they run one after
     // the other.  Same arithmetic either way.
@@ -653,6 +738,8 @@ __global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__r
                                                               zc *__restrict__ hh_tau, uint32_t *__restrict__ prog)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    extern __shared__ __align__(16) unsigned char zsm_td[];      // packed triangle of the diagonal block + NBW dots
+    zc *TD = reinterpret_cast<zc *>(zsm_td);
     __shared__ zc v[NBW], p[NBW], w2[NBW], zsc[2];
     __shared__ double dsc[1];
     const int tid = threadIdx.x;
@@ -673,7 +760,7 @@ __global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__r
                 __syncthreads();
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
-            bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head);
+            bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc, head + s, head + s - 1, need_head, TD);
             // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
             // barriers are built from): one fence, not one per thread
             __syncthreads();
@@ -1019,8 +1106,12 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
             cudaError_t e0 = set_max_smem((const void *)zk, zbytes);
             if (e0 != cudaSuccess) return e0;
             e1 = bc_launch_persistent(zk, grid, 256, zbytes, st, N, ab, hh_v, hh_tau, prog);
-        } else
-            e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 384, 0, st, N, ab, hh_v, hh_tau, prog);
+        } else {
+            constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW) * 16;       // triangle of block (ii) + NBW dot products
+            cudaError_t e0 = set_max_smem((const void *)bc_persistent_kernel_z<NBW>, tbytes);
+            if (e0 != cudaSuccess) return e0;
+            e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 384, tbytes, st, N, ab, hh_v, hh_tau, prog);
+        }
         ++nl;
         if (e1 != cudaSuccess) return e1;
     } else if (N >= 2) {
