@@ -26,8 +26,13 @@ template <int NBW>
 __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s, const int64_t k, double *__restrict__ ab,
                                                double *__restrict__ hh_v, double *__restrict__ hh_tau, double *v, double *p,
                                                double *w2, double *red, double *sc, uint32_t *head_mine = nullptr,
-                                               const uint32_t *head_prev = nullptr, const uint32_t need_head = 0)
+                                               const uint32_t *head_prev = nullptr, const uint32_t need_head = 0,
+                                               double *TD = nullptr)
 {
+    // TD != nullptr (persistent kernel, 384 threads): shared memory for the packed lower triangle of the
+    // diagonal block + NBW dot products; see bc_step_global_z
+    constexpr int TRI = NBW * (NBW + 1) / 2;
+    auto toff = [](int j) { return j * NBW - ((j * (j - 1)) >> 1); };
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
     constexpr int64_t ldab = 2 * NBW + 1;
     const int tid = threadIdx.x, nt = blockDim.x;
@@ -46,6 +51,14 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
             if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
         }
         return;
+    }
+    if (TD) {
+        for (int j = tid >> 5; j < L; j += nt >> 5) {
+            const double *src = &BC_B(r0 + j, r0 + j);
+            double *dst = TD + toff(j);
+            for (int i = tid & 31; i < L - j; i += 32) cp_async8(smem_u32(dst + i), src + i, 8u);
+        }
+        cp_async_commit();
     }
     // --- Householder generator (R7): beta = -sign(alpha) ||x||, tau = (beta - alpha)/beta, v = x/(alpha - beta)
     if (tid < L) p[tid] = BC_B(r0 + tid, c);     // x, parked in p
@@ -80,7 +93,68 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
         hh_tau[g] = tau;
         if (head_mine) asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(head_mine), "r"((uint32_t)(k + 1)) : "memory");
     }
+    if (TD) {
+        cp_async_wait_all();
+        __syncthreads();
+    }
     if (tau == 0.0) return;
+    if (TD) {
+        const int grp = tid >> 7, t0 = tid & 127;
+        double *dA = TD + TRI;
+#define DD(i, j) (((i) >= (j)) ? TD[toff(j) + (i) - (j)] : TD[toff(i) + (j) - (i)])
+        if (grp == 0) {
+            for (int64_t j = c + 1 + t0; j < r0; j += 128) {
+                double dot = 0.0;
+                for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BC_B(r0 + i, j)));
+                dA[j - (c + 1)] = dot;
+            }
+        } else if (grp == 1) {
+            int64_t r2 = r1 + NBW;
+            if (r2 > N - 1) r2 = N - 1;
+            for (int64_t i = r1 + 1 + t0; i <= r2; i += 128) {
+                if (need_head && i == r2) {      // the corner is the head element of step (s-1, k+2): wait for its beta
+                    uint32_t h;
+                    do {
+                        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
+                    } while (h < need_head);
+                }
+                double dot = 0.0;
+                for (int l = 0; l < L; ++l) dot = __dadd_rn(dot, __dmul_rn(BC_B(i, r0 + l), v[l]));
+                for (int l = 0; l < L; ++l) BC_B(i, r0 + l) = __dsub_rn(BC_B(i, r0 + l), __dmul_rn(__dmul_rn(tau, dot), v[l]));
+            }
+        } else {
+            for (int j = t0; j < L; j += 128) {
+                double dot = 0.0;
+#pragma unroll 8
+                for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], DD(i, j)));
+                red[j] = dot;
+            }
+            asm volatile("bar.sync 1, 128;" ::: "memory");
+            for (int i = t0; i < L; i += 128) {
+                double dot = 0.0;
+#pragma unroll 8
+                for (int j = 0; j < L; ++j) {
+                    const double m = __dsub_rn(DD(i, j), __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+                    dot = __dadd_rn(dot, __dmul_rn(m, v[j]));
+                }
+                w2[i] = dot;
+            }
+        }
+        __syncthreads();
+        {
+            const int ty = tid >> 7, i = tid & 127;
+            if (i < L) {
+                for (int64_t j = c + 1 + ty; j < r0; j += 3)
+                    BC_B(r0 + i, j) = __dsub_rn(BC_B(r0 + i, j), __dmul_rn(__dmul_rn(tau, v[i]), dA[j - (c + 1)]));
+                for (int j = ty; j <= i; j += 3) {
+                    const double m = __dsub_rn(TD[toff(j) + i - j], __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
+                    BC_B(r0 + i, r0 + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
+                }
+            }
+        }
+#undef DD
+        return;
+    }
     // 384 threads (persistent kernel): three groups of 128 run (i), (iii), (ii) side by side; see bc_step_global_z
     const bool par = nt >= 384;
     const int grp = par ? (tid >> 7) : 0, t0 = par ? (tid & 127) : tid, st_ = par ? 128 : nt;
@@ -164,6 +238,7 @@ __global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, do
                                                                    uint32_t *__restrict__ prog)
 {
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
+    extern __shared__ double td_smem[];                // packed triangle of the diagonal block + NBW dots
     __shared__ double v[NBW], p[NBW], w2[NBW], red[128], sc[3];
     const int tid = threadIdx.x;
     uint32_t *done = prog, *head = prog + N;
@@ -183,7 +258,7 @@ __global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, do
                 __syncthreads();
                 if (k + 2 < Kprev) need_head = (uint32_t)(k + 3);
             }
-            bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc, head + s, head + s - 1, need_head);
+            bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc, head + s, head + s - 1, need_head, td_smem);
             // the CTA barrier orders every thread's stores before thread 0's release (the pattern grid-wide
             // barriers are built from): one fence, not one per thread
             __syncthreads();
@@ -1042,7 +1117,10 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     }
     if (NBW > 64 && prog && nsm > 0 && N >= 2) {
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 384, 0, st, N, ab, hh_v, hh_tau, prog);
+        constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW) * 8;          // triangle of block (ii) + NBW dot products
+        cudaError_t e0 = set_max_smem((const void *)bc_persistent_global_kernel<NBW>, tbytes);
+        if (e0 != cudaSuccess) return e0;
+        cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 384, tbytes, st, N, ab, hh_v, hh_tau, prog);
         ++nl;
         if (e1 != cudaSuccess) return e1;
     } else if (NBW <= 64 && prog && nsm > 0 && N >= 2) {
