@@ -30,7 +30,8 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
                                                double *TD = nullptr)
 {
     // TD != nullptr (persistent kernel, 384 threads): shared memory for the packed lower triangle of the
-    // diagonal block + NBW dot products; see bc_step_global_z
+    // diagonal block + NBW dot products + the tile of block (i) (real: both fit, 196 KB at nbw = 128; block
+    // (iii), whose accesses are coalesced anyway, stays in global memory); see bc_step_global_z
     constexpr int TRI = NBW * (NBW + 1) / 2;
     auto toff = [](int j) { return j * NBW - ((j * (j - 1)) >> 1); };
     constexpr int LG = (NBW == 32) ? 5 : (NBW == 64) ? 6 : 7;
@@ -52,11 +53,18 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
         }
         return;
     }
+    constexpr int LDA = NBW + 1;                       // column stride of the block (i) tile
+    double *TA = TD ? TD + TRI + NBW : nullptr;        // block (i): column q = matrix column c+1+q, rows r0 ..
     if (TD) {
         for (int j = tid >> 5; j < L; j += nt >> 5) {
             const double *src = &BC_B(r0 + j, r0 + j);
             double *dst = TD + toff(j);
             for (int i = tid & 31; i < L - j; i += 32) cp_async8(smem_u32(dst + i), src + i, 8u);
+        }
+        for (int64_t j = c + 1 + (tid >> 5); j < r0; j += nt >> 5) {
+            const double *src = &BC_B(r0, j);
+            double *dst = TA + (j - (c + 1)) * LDA;
+            for (int i = tid & 31; i < L; i += 32) cp_async8(smem_u32(dst + i), src + i, 8u);
         }
         cp_async_commit();
     }
@@ -104,8 +112,10 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
 #define DD(i, j) (((i) >= (j)) ? TD[toff(j) + (i) - (j)] : TD[toff(i) + (j) - (i)])
         if (grp == 0) {
             for (int64_t j = c + 1 + t0; j < r0; j += 128) {
+                const double *col = TA + (j - (c + 1)) * LDA;
                 double dot = 0.0;
-                for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], BC_B(r0 + i, j)));
+#pragma unroll 8
+                for (int i = 0; i < L; ++i) dot = __dadd_rn(dot, __dmul_rn(v[i], col[i]));
                 dA[j - (c + 1)] = dot;
             }
         } else if (grp == 1) {
@@ -145,7 +155,7 @@ __device__ __forceinline__ void bc_step_global(const int64_t N, const int64_t s,
             const int ty = tid >> 7, i = tid & 127;
             if (i < L) {
                 for (int64_t j = c + 1 + ty; j < r0; j += 3)
-                    BC_B(r0 + i, j) = __dsub_rn(BC_B(r0 + i, j), __dmul_rn(__dmul_rn(tau, v[i]), dA[j - (c + 1)]));
+                    BC_B(r0 + i, j) = __dsub_rn(TA[(j - (c + 1)) * LDA + i], __dmul_rn(__dmul_rn(tau, v[i]), dA[j - (c + 1)]));
                 for (int j = ty; j <= i; j += 3) {
                     const double m = __dsub_rn(TD[toff(j) + i - j], __dmul_rn(__dmul_rn(tau, v[i]), red[j]));
                     BC_B(r0 + i, r0 + j) = __dsub_rn(m, __dmul_rn(__dmul_rn(tau, w2[i]), v[j]));
@@ -1117,7 +1127,8 @@ cudaError_t launch_bulge_chase(int64_t N, double *ab, double *hh_v, double *hh_t
     }
     if (NBW > 64 && prog && nsm > 0 && N >= 2) {
         const int64_t grid = (N - 1 < nsm) ? N - 1 : nsm;
-        constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW) * 8;          // triangle of block (ii) + NBW dot products
+        // triangle of block (ii) + NBW dot products + the tile of block (i)
+        constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW + (NBW - 1) * (NBW + 1)) * 8;
         cudaError_t e0 = set_max_smem((const void *)bc_persistent_global_kernel<NBW>, tbytes);
         if (e0 != cudaSuccess) return e0;
         cudaError_t e1 = bc_launch_persistent(bc_persistent_global_kernel<NBW>, grid, 384, tbytes, st, N, ab, hh_v, hh_tau, prog);
