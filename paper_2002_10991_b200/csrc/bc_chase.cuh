@@ -679,11 +679,41 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
         zc *dA = TD + TRI;
 #define DZ(i, j) (((i) >= (j)) ? TD[toff(j) + (i) - (j)] : zconj(TD[toff(i) + (j) - (i)]))
         if (grp == 0) {
-            // --- (i), first half: the dot products v^H A, one thread per column
-            for (int64_t j = c + 1 + t0; j < r0; j += 128) {
+            // --- (i), first half: the dot products v^H A, one thread per column.  The block (260 KB) does not fit
+            //     beside the triangle, so it passes through shared memory 16 rows at a time (two buffers,
+            //     [column][17 elements]): the copies are coalesced (16 lanes along the 256 contiguous bytes of
+            //     a column) and the next chunk is in flight while this one is summed, in the definition's order
+            const int nA = (int)(r0 - c - 1);
+            if (nA > 0) {
+                zc *CH = TD + TRI + NBW;
+                constexpr int CS = 17, CB = (NBW - 1) * CS;
+                const int nch = (L + 15) >> 4;
+                auto fetch = [&](int ch, int buf) {
+                    const int i = 16 * ch + (t0 & 15);
+                    for (int q = t0 >> 4; q < nA; q += 8)
+                        cp_async16(smem_u32(CH + buf * CB + q * CS + (t0 & 15)), &BC_Z(r0 + (i < L ? i : 0), c + 1 + q),
+                                   i < L ? 16u : 0u);
+                    cp_async_commit();
+                };
+                fetch(0, 0);
                 zc dot = {0.0, 0.0};
-                for (int i = 0; i < L; ++i) dot = zadd(dot, zmul(zconj(v[i]), BC_Z(r0 + i, j)));
-                dA[j - (c + 1)] = dot;
+                for (int ch = 0; ch < nch; ++ch) {
+                    if (ch + 1 < nch) {
+                        fetch(ch + 1, (ch + 1) & 1);
+                        asm volatile("cp.async.wait_group 1;" ::: "memory");
+                    } else {
+                        asm volatile("cp.async.wait_group 0;" ::: "memory");
+                    }
+                    asm volatile("bar.sync 2, 128;" ::: "memory");
+                    if (t0 < nA) {
+                        const zc *col = CH + (ch & 1) * CB + t0 * CS;
+#pragma unroll
+                        for (int r = 0; r < 16; ++r)
+                            if (16 * ch + r < L) dot = zadd(dot, zmul(zconj(v[16 * ch + r]), col[r]));
+                    }
+                    asm volatile("bar.sync 2, 128;" ::: "memory");      // the buffer may be refilled
+                }
+                if (t0 < nA) dA[t0] = dot;
             }
         } else if (grp == 1) {
             // --- (iii) E <- E H = E - tau (E v) v^H, one thread per row (coalesced both ways)
@@ -1196,7 +1226,8 @@ cudaError_t launch_bulge_chase_z(int64_t N, zc *ab, zc *hh_v, zc *hh_tau, double
             if (e0 != cudaSuccess) return e0;
             e1 = bc_launch_persistent(zk, grid, 256, zbytes, st, N, ab, hh_v, hh_tau, prog);
         } else {
-            constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW) * 16;       // triangle of block (ii) + NBW dot products
+            // triangle of block (ii) + NBW dot products + two 16-row chunk buffers of block (i)
+            constexpr int tbytes = (NBW * (NBW + 1) / 2 + NBW + 2 * (NBW - 1) * 17) * 16;
             cudaError_t e0 = set_max_smem((const void *)bc_persistent_kernel_z<NBW>, tbytes);
             if (e0 != cudaSuccess) return e0;
             e1 = bc_launch_persistent(bc_persistent_kernel_z<NBW>, grid, 384, tbytes, st, N, ab, hh_v, hh_tau, prog);
