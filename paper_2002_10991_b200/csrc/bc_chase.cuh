@@ -726,9 +726,27 @@ __device__ __forceinline__ void bc_step_global_z(const int64_t N, const int64_t 
                         asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(h) : "l"(head_prev) : "memory");
                     } while (h < need_head);
                 }
+                // (eight loads in flight at a time -- the row's elements are 4 KB apart; the sum keeps its order)
                 zc dot = {0.0, 0.0};
-                for (int l = 0; l < L; ++l) dot = zadd(dot, zmul(BC_Z(i, r0 + l), v[l]));
-                for (int l = 0; l < L; ++l) BC_Z(i, r0 + l) = zsub(BC_Z(i, r0 + l), zmul(zmul(tau, dot), zconj(v[l])));
+                for (int l0 = 0; l0 < L; l0 += 8) {
+                    zc e[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (l0 + u < L) e[u] = BC_Z(i, r0 + l0 + u);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (l0 + u < L) dot = zadd(dot, zmul(e[u], v[l0 + u]));
+                }
+                const zc td = zmul(tau, dot);
+                for (int l0 = 0; l0 < L; l0 += 8) {
+                    zc e[8];
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (l0 + u < L) e[u] = BC_Z(i, r0 + l0 + u);
+#pragma unroll
+                    for (int u = 0; u < 8; ++u)
+                        if (l0 + u < L) BC_Z(i, r0 + l0 + u) = zsub(e[u], zmul(td, zconj(v[l0 + u])));
+                }
             }
         } else {
             // --- (ii), first two phases, out of shared memory: p = v^H D;  w2 = (D - conj(tau) v p) v
