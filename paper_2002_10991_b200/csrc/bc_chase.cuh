@@ -241,7 +241,8 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel(int64_t N, int64_t t,
     bc_step_global<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, red, sc);
 }
 
-// persistent version of the global-memory step (used for nbw = 128): flags and 2-step lag as in
+// persistent version of the nbw = 128 step (block (ii) and, real, block (i) in shared memory; see TD in
+// bc_step_global): flags and 2-step lag as in
 // bc_persistent_kernel below
 template <int NBW>
 __global__ void __launch_bounds__(384) bc_persistent_global_kernel(int64_t N, double *__restrict__ ab,
@@ -874,7 +875,8 @@ __global__ void __launch_bounds__(128) bc_wavefront_kernel_z(int64_t N, int64_t 
     bc_step_global_z<NBW>(N, s, k, ab, hh_v, hh_tau, v, p, w2, zsc, dsc);
 }
 
-// persistent complex version: same flags and 2-step lag as bc_persistent_kernel, step on global memory
+// persistent complex version (nbw = 128): same flags and 2-step lag as bc_persistent_kernel; block (ii) in
+// shared memory, block (i) streamed through it (TD in bc_step_global_z)
 template <int NBW>
 __global__ void __launch_bounds__(384) bc_persistent_kernel_z(int64_t N, zc *__restrict__ ab, zc *__restrict__ hh_v,
                                                               zc *__restrict__ hh_tau, uint32_t *__restrict__ prog)
