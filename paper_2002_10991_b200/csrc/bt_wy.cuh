@@ -564,11 +564,14 @@ inline double wy_smsp_load(int P, int64_t n)
     for (int s = 0; s < 4; ++s) mx = load[s] > mx ? load[s] : mx;
     return mx;
 }
-// Real kernel, one wave: the P in {1, 2, 4} that balances the sub-partitions (partial spectra, PAPER.md:218:
-// 5-16 slabs per SM).  Measured on B200 (N = 8192, nbw 64, n slabs per SM; TFLOP/s for P = 1 / 2 / 4):
-// n = 5: 15.3 / 19.8 / 25.9, 6: 18.8 / 23.7 / 26.9, 7: 22.3 / 23.6 / 27.1, 9: 21.0 / 25.7 / -, 10: 23.2 / 28.4 / -,
-// 13: 24.2 / 26.7 / -.  Up to 8 slabs P = 4 always wins (one-slab warps two to a sub-partition run the pipe
-// badly); above that P = 2 when it lowers the busiest sub-partition by more than its 3 % hand-over cost.
+// Real kernel, one wave: P in {1, 2, 4} for partial spectra (5-16 slabs per SM).  Measured on B200
+// (N = 8192, nbw 64, n slabs per SM; TFLOP/s for P = 1 / 2 / 4):
+//   n = 5: 15.3 / 19.8 / 25.9    6: 18.8 / 23.7 / 26.9    7: 22.3 / 23.6 / 27.1
+//   n = 9: 21.0 / 25.7    10: 23.2 / 28.4    11: 25.5 / 27.9    12: 27.8 / 29.8    13: 24.2 / 26.7    14: 26.0 / 28.7
+//   n = 15: 27.8 / 27.5   16: 29.6 / 29.4
+// Two things are at work: the balance of the four sub-partitions (wy_smsp_load) and the number of slabs a
+// warp holds -- warps with 3-4 slabs run the DMMA pipe better than warps with 1-2, and P warps that share a
+// group of slabs hold P times as many each.  Hence: up to 8 slabs P = 4, 9-14 slabs P = 2, above that P = 1.
 inline int wy_pick_P_real(int64_t nslab, int64_t K0, int nsm, int ngmax, int maxP)
 {
     const int64_t grid = nslab < nsm ? nslab : nsm;
@@ -576,6 +579,7 @@ inline int wy_pick_P_real(int64_t nslab, int64_t K0, int nsm, int ngmax, int max
     if (n > 8 * (int64_t)ngmax) return 1;              // more than one wave of the P = 1 launch
     auto ok = [&](int P) { return P <= maxP && 4 * P <= K0 && n <= (int64_t)(8 / P) * ngmax; };
     if (n <= 8) return ok(4) ? 4 : ok(2) ? 2 : 1;
+    if (n <= 14) return ok(2) ? 2 : 1;
     return (ok(2) && wy_smsp_load(2, n) * 1.03 < wy_smsp_load(1, n)) ? 2 : 1;
 }
 

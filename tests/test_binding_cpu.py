@@ -152,7 +152,7 @@ def test_launch_plan_balances_sub_partitions_for_partial_spectra():
     """PAPER.md:218 (KS-DFT: 20-69 % of the eigenvectors): 5-16 slabs per SM.  The plan picks the number of
     warps per slab group that balances the four sub-partitions (measured table there)."""
     N, nbw = 32768, 64
-    for frac, P in ((0.2, 4), (0.25, 4), (0.4, 1), (0.35, 2), (0.45, 2), (0.6, 1), (0.69, 1), (1.0, 1)):
+    for frac, P in ((0.2, 4), (0.25, 4), (0.4, 2), (0.35, 2), (0.45, 2), (0.5, 2), (0.6, 1), (0.69, 1), (1.0, 1)):
         nev = int(round(frac * N))
         pl = binding.plan(False, N, nbw, nev, 148)
         assert pl["P"] == P and pl["grid"] == 148 and pl["warps_per_cta"] == 8, (frac, pl)

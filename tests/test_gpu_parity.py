@@ -98,7 +98,7 @@ def test_chain_parallel_mode(nbw, cplx):
     _check(12 * nbw + 7, nbw, 148 * 8 * 3 + 5, cplx)   # 3-4 slabs per CTA: P = 2, ragged tail
 
 
-@pytest.mark.parametrize("nbw,n", [(32, 5), (64, 6), (64, 7), (64, 10), (64, 13), (128, 3), (128, 7), (96, 4)])
+@pytest.mark.parametrize("nbw,n", [(32, 5), (64, 6), (64, 7), (64, 10), (64, 12), (64, 13), (64, 14), (128, 3), (128, 7), (96, 4)])
 def test_partial_spectrum_plans(nbw, n):
     # 5-16 slabs per CTA: the plan shares slab groups among P = 4 / 2 warps with SEVERAL slabs per warp
     # (the sub-partition balance of DESIGN.md 5.1); ragged last slab
